@@ -1,0 +1,123 @@
+/*
+ * sparse_attn.h -- C ABI of the B200 (sm_100a) tile-skipping attention forward pass.
+ *
+ * One hot path of arxiv/paper_2606_16317 ("Training-Free Sparse Attention Based on Cumulative
+ * Energy Filtering"): a FlashAttention-style forward pass for non-causal self-attention that
+ * decides, inside the K-tile loop and from the online-softmax statistics only, whether a
+ * (Q_i, K_j) tile is skipped (section 3.1, Eq. 5-6).  No mask pre-pass.
+ *
+ * All entry points are plain C, never throw, never exit the process, and allocate no persistent
+ * device memory.  There is no CPU fallback: on a machine without an sm_100 device every compute
+ * call fails with SPARSE_ATTN_ERR_DEVICE.
+ */
+#ifndef SPARSE_ATTN_H_
+#define SPARSE_ATTN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPARSE_ATTN_VERSION 100 /* 0.1.0 */
+
+/* mode argument of sparse_attn_fwd */
+enum sparse_attn_mode {
+    SPARSE_ATTN_DENSE = 0,   /* no skipping: softmax(scale * Q K^T) V, FlashAttention-2 tiling */
+    SPARSE_ATTN_FIXED = 1,   /* BLASST-style: skip tile j iff  mhat_r - m_r^(j-1) < lambda  for every valid row r
+                                (tile max minus running max over retained tiles) */
+    SPARSE_ATTN_DYNAMIC = 2  /* DynSparse: skip tile j iff  t_r = mhat_r - LSE_r^(j-1) < lambda  for every valid row r,
+                                LSE over the retained tiles only (Eq. 5-6) */
+};
+
+/* return codes: 0 on success, negative on error */
+enum sparse_attn_status {
+    SPARSE_ATTN_OK = 0,
+    SPARSE_ATTN_ERR_NULL_POINTER = -1, /* a required pointer is NULL */
+    SPARSE_ATTN_ERR_SHAPE = -2,        /* B, H or N <= 0, or B*H / N too large for the launch */
+    SPARSE_ATTN_ERR_HEAD_DIM = -3,     /* D not in {64, 128} */
+    SPARSE_ATTN_ERR_TILE = -4,         /* tile_q / tile_k not the supported decision tile for this D */
+    SPARSE_ATTN_ERR_MODE = -5,         /* mode not in {0, 1, 2} */
+    SPARSE_ATTN_ERR_PARAMS = -6,       /* params NULL in a sparse mode, struct_size wrong, lambda NaN,
+                                          lambda > 0 in FIXED mode, softmax_scale negative / non-finite */
+    SPARSE_ATTN_ERR_ALIGNMENT = -7,    /* q, k, v or out not 16-byte aligned (TMA / vector stores) */
+    SPARSE_ATTN_ERR_DEVICE = -8,       /* no CUDA device, or the current device is not sm_100 (B200) */
+    SPARSE_ATTN_ERR_CUDA = -9          /* a CUDA runtime / driver call failed; see sparse_attn_last_error() */
+};
+
+/*
+ * Threshold and launch parameters.  Host struct, plain C; the first field versions it.
+ */
+typedef struct sparse_attn_params {
+    uint32_t struct_size;   /* must be sizeof(sparse_attn_params) */
+    float lambda;           /* threshold lambda of PAPER.md:123, natural-log logit units (S includes the softmax
+                               scale).  A tile is skipped iff max over its valid rows of t_r is < lambda (strict).
+                               -INFINITY disables skipping.  In FIXED mode it is ln(alpha) and must be <= 0. */
+    float softmax_scale;    /* 0 means 1/sqrt(D) */
+    int32_t tile_q;         /* decision tile rows B_r; 0 = default (64 for D = 64, 128 for D = 128) */
+    int32_t tile_k;         /* decision tile columns B_c; 0 = default (same as tile_q) */
+    void* stream;           /* cudaStream_t to launch on; NULL = the default stream */
+    uint8_t* skip_mask_out; /* optional, device, [B, H, T_r, T_c] bytes, 1 = tile skipped, fully overwritten.
+                               T_r = ceil(N / tile_q), T_c = ceil(N / tile_k).  NULL in timed runs. */
+    float* margin_out;      /* optional, device, [B, H, T_r, T_c] fp32: g_ij = max_r t_r - lambda as evaluated on
+                               the GPU (+inf for tile 0 and in DENSE mode).  Debug / parity only. */
+} sparse_attn_params;
+
+/*
+ * Forward pass.  Enqueues work on params->stream (or the default stream) and returns; the caller
+ * synchronises.  One GPU, the current device.
+ *
+ *   q, k, v  device, bf16, [B, H, N, D] contiguous, 16-byte aligned, never written
+ *   out      device, bf16, [B, H, N, D]; fully overwritten.  Rows are renormalised over the retained
+ *            tiles (Eq. 1): out_r = sum_{c in retained tiles} e^{S_rc - lse_r} v_c
+ *   lse      device, fp32, [B, H, N], natural log, over the retained tiles (Eq. 6); may be NULL
+ *   B,H,N,D  batch, heads, tokens (N_q = N_k, non-causal), head dim in {64, 128}
+ *   params   host pointer; may be NULL only when mode == SPARSE_ATTN_DENSE
+ *   mode     enum sparse_attn_mode
+ *   stats_out device, int64, [B, H, 2] = {executed, skipped} decision-tile counts per head
+ *            (executed + skipped = T_r * T_c; "Sps"); overwritten; may be NULL
+ *
+ * K tiles are visited in ascending token order for every Q tile (decisions are order dependent);
+ * tile j = 0 is never skipped; a skipped tile leaves m, l and O untouched; Q K^T is computed for
+ * every tile, exp / row-sum / P V only for retained ones.
+ *
+ * Returns SPARSE_ATTN_OK or a negative sparse_attn_status; arguments are validated on the host
+ * before anything is launched, so on error nothing has been written.
+ */
+int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, float* lse,
+                    int B, int H, int N, int D,
+                    const sparse_attn_params* params, int mode, int64_t* stats_out);
+
+/*
+ * Same operation with HOST buffers (pageable or pinned): allocates device scratch, copies q, k, v
+ * host->device, runs sparse_attn_fwd, copies out / lse / stats back, synchronises and frees.
+ * params->skip_mask_out / margin_out, if set, are host pointers here too.  Used for end-to-end
+ * timing; layouts as above.
+ */
+int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse,
+                         int B, int H, int N, int D,
+                         const sparse_attn_params* params, int mode, int64_t* stats_out);
+
+/* lambda = ln((1 - recall) / N): the worst-case threshold under which every row keeps more than
+ * `recall` of its softmax mass (lambda = ln(eps / L)).  Pure host function. */
+double sparse_attn_lambda_from_recall(double recall, int N);
+
+/* lambda = ln(p_real) + ln(tile_k / N)  (Eq. 7).  Pure host function. */
+double sparse_attn_lambda_from_preal(double p_real, int tile_k, int N);
+
+/* Static string for a status code. */
+const char* sparse_attn_status_string(int status);
+
+/* Detail of the last error on this thread ("" if none).  Valid until the next call on the thread. */
+const char* sparse_attn_last_error(void);
+
+/* SPARSE_ATTN_VERSION of the loaded library. */
+int sparse_attn_version(void);
+
+/* Number of kernel launches sparse_attn_fwd has enqueued in this process (for bench accounting). */
+int64_t sparse_attn_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPARSE_ATTN_H_ */

@@ -1,0 +1,23 @@
+"""B200 (sm_100a) tile-skipping attention forward of arxiv/paper_2606_16317 (DynSparse).
+
+Thin ctypes binding over the C ABI in include/sparse_attn.h; every step of the hot path runs in
+the CUDA kernels of csrc/.  There is no CPU fallback: compute calls raise on a machine without
+the built extension or without an sm_100 device.
+"""
+from .binding import (  # noqa: F401
+    MODE_DENSE,
+    MODE_DYNAMIC,
+    MODE_FIXED,
+    SparseAttnError,
+    SparseAttnParams,
+    lambda_from_preal,
+    lambda_from_recall,
+    last_error,
+    launch_count,
+    library_path,
+    make_params,
+    sparse_attn_fwd,
+    sparse_attn_fwd_host,
+    status_string,
+    version,
+)

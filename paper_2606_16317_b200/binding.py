@@ -1,0 +1,156 @@
+"""ctypes binding of include/sparse_attn.h -- argument marshalling only.
+
+`sparse_attn_fwd` takes torch CUDA tensors (torch is used for device memory and streams, nothing
+else) or raw device pointers, and calls the C entry point of the same name.  The extension must
+have been built (`python -m paper_2606_16317_b200.build` or `__graft_entry__.build()`); loading
+fails loudly otherwise -- there is no fallback path.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+MODE_DENSE, MODE_FIXED, MODE_DYNAMIC = 0, 1, 2
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libsparse_attn.so")
+_lib = None
+
+# every symbol include/sparse_attn.h declares
+EXPORTED_SYMBOLS = (
+    "sparse_attn_fwd",
+    "sparse_attn_fwd_host",
+    "sparse_attn_lambda_from_recall",
+    "sparse_attn_lambda_from_preal",
+    "sparse_attn_status_string",
+    "sparse_attn_last_error",
+    "sparse_attn_version",
+    "sparse_attn_launch_count",
+)
+
+
+class SparseAttnError(RuntimeError):
+    def __init__(self, status: int, detail: str):
+        super().__init__(f"sparse_attn status {status} ({status_string(status)}): {detail}")
+        self.status = status
+        self.detail = detail
+
+
+class SparseAttnParams(ctypes.Structure):
+    """Mirror of `sparse_attn_params` (include/sparse_attn.h)."""
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32),
+        ("lambda_", ctypes.c_float),
+        ("softmax_scale", ctypes.c_float),
+        ("tile_q", ctypes.c_int32),
+        ("tile_k", ctypes.c_int32),
+        ("stream", ctypes.c_void_p),
+        ("skip_mask_out", ctypes.c_void_p),
+        ("margin_out", ctypes.c_void_p),
+    ]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(
+                f"{_LIB_PATH} is missing: build the CUDA extension first "
+                "(python -m paper_2606_16317_b200.build). There is no CPU fallback.")
+        lib = ctypes.CDLL(_LIB_PATH)
+        fwd_args = [ctypes.c_void_p] * 5 + [ctypes.c_int] * 4 + [ctypes.POINTER(SparseAttnParams), ctypes.c_int,
+                                                                 ctypes.c_void_p]
+        lib.sparse_attn_fwd.restype = ctypes.c_int
+        lib.sparse_attn_fwd.argtypes = fwd_args
+        lib.sparse_attn_fwd_host.restype = ctypes.c_int
+        lib.sparse_attn_fwd_host.argtypes = fwd_args
+        lib.sparse_attn_lambda_from_recall.restype = ctypes.c_double
+        lib.sparse_attn_lambda_from_recall.argtypes = [ctypes.c_double, ctypes.c_int]
+        lib.sparse_attn_lambda_from_preal.restype = ctypes.c_double
+        lib.sparse_attn_lambda_from_preal.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int]
+        lib.sparse_attn_status_string.restype = ctypes.c_char_p
+        lib.sparse_attn_status_string.argtypes = [ctypes.c_int]
+        lib.sparse_attn_last_error.restype = ctypes.c_char_p
+        lib.sparse_attn_last_error.argtypes = []
+        lib.sparse_attn_version.restype = ctypes.c_int
+        lib.sparse_attn_launch_count.restype = ctypes.c_int64
+        _lib = lib
+    return _lib
+
+
+def version() -> int:
+    return _load().sparse_attn_version()
+
+
+def launch_count() -> int:
+    return _load().sparse_attn_launch_count()
+
+
+def status_string(status: int) -> str:
+    return _load().sparse_attn_status_string(int(status)).decode()
+
+
+def last_error() -> str:
+    return _load().sparse_attn_last_error().decode()
+
+
+def lambda_from_recall(recall: float, N: int) -> float:
+    return _load().sparse_attn_lambda_from_recall(float(recall), int(N))
+
+
+def lambda_from_preal(p_real: float, tile_k: int, N: int) -> float:
+    return _load().sparse_attn_lambda_from_preal(float(p_real), int(tile_k), int(N))
+
+
+def _ptr(x) -> Optional[int]:
+    """Device/host address of a torch tensor, numpy array, int or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "ctypes"):
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def make_params(lam: float = float("-inf"), softmax_scale: float = 0.0, tile_q: int = 0, tile_k: int = 0,
+                stream=None, skip_mask_out=None, margin_out=None) -> SparseAttnParams:
+    p = SparseAttnParams()
+    p.struct_size = ctypes.sizeof(SparseAttnParams)
+    p.lambda_ = lam
+    p.softmax_scale = softmax_scale
+    p.tile_q = tile_q
+    p.tile_k = tile_k
+    p.stream = _ptr(stream)
+    p.skip_mask_out = _ptr(skip_mask_out)
+    p.margin_out = _ptr(margin_out)
+    return p
+
+
+def _call(fn, q, k, v, out, lse, B, H, N, D, params, mode, stats_out):
+    rc = fn(_ptr(q), _ptr(k), _ptr(v), _ptr(out), _ptr(lse), int(B), int(H), int(N), int(D),
+            ctypes.byref(params) if params is not None else None, int(mode), _ptr(stats_out))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_fwd(q, k, v, out, lse, B, H, N, D, threshold_params, mode, stats_out):
+    """C entry point `sparse_attn_fwd` (device buffers).  Tensors or raw pointers; see the header.
+
+    Enqueues on threshold_params.stream (torch's current stream if the caller passed it there) and
+    returns; the caller synchronises.
+    """
+    return _call(_load().sparse_attn_fwd, q, k, v, out, lse, B, H, N, D, threshold_params, mode, stats_out)
+
+
+def sparse_attn_fwd_host(q, k, v, out, lse, B, H, N, D, threshold_params, mode, stats_out):
+    """C entry point `sparse_attn_fwd_host` (host buffers; copies inside, synchronous)."""
+    return _call(_load().sparse_attn_fwd_host, q, k, v, out, lse, B, H, N, D, threshold_params, mode, stats_out)

@@ -1,0 +1,269 @@
+// C-ABI of the tile-skipping attention forward (include/sparse_attn.h): argument validation,
+// TMA tensor maps, launch.  No CPU fallback: without an sm_100 device every compute call fails.
+#include "../../include/sparse_attn.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "fwd_kernel.cuh"
+
+namespace {
+
+thread_local char g_last_error[512] = "";
+std::atomic<int64_t> g_launches{0};
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_last_error, sizeof g_last_error, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                           \
+    do {                                                                                         \
+        cudaError_t err__ = (expr);                                                              \
+        if (err__ != cudaSuccess)                                                                \
+            return fail(SPARSE_ATTN_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(err__)); \
+    } while (0)
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int get_encode_fn(EncodeTiledFn* out) {
+    static EncodeTiledFn cached = nullptr;
+    if (!cached) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !fn)
+            return fail(SPARSE_ATTN_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
+        cached = reinterpret_cast<EncodeTiledFn>(fn);
+    }
+    *out = cached;
+    return 0;
+}
+
+// bf16 [BH, N, D] tensor, box = 64 columns (128 B, SWIZZLE_128B) x `rows` tokens of one head.
+// Out-of-range tokens (ragged last tile) are zero-filled by TMA and never bleed into the next head.
+int make_tmap(EncodeTiledFn enc, CUtensorMap* tm, const void* base, int BH, int N, int D, int rows) {
+    cuuint64_t dims[3] = {static_cast<cuuint64_t>(D), static_cast<cuuint64_t>(N), static_cast<cuuint64_t>(BH)};
+    cuuint64_t strides[2] = {static_cast<cuuint64_t>(D) * 2, static_cast<cuuint64_t>(N) * D * 2};
+    cuuint32_t box[3] = {64, static_cast<cuuint32_t>(rows), 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(SPARSE_ATTN_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return 0;
+}
+
+template <int D, int BC, int G, int NSTAGE>
+int launch(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const dsa::FwdArgs& args, int BH,
+           cudaStream_t stream) {
+    using L = dsa::SmemLayout<D, BC, NSTAGE>;
+    auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NSTAGE>;
+    static bool configured = false;
+    if (!configured) {
+        CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L::kDynamicBytes));
+        configured = true;
+    }
+    dim3 grid((args.n_mma_tiles + 1) / 2, BH, 1);
+    kernel<<<grid, dsa::kNumThreads, L::kDynamicBytes, stream>>>(tq, tk, tv, args);
+    CUDA_TRY(cudaGetLastError());
+    g_launches.fetch_add(1);
+    return 0;
+}
+
+struct Resolved {
+    int tile_q, tile_k;
+    float scale, lambda;
+    cudaStream_t stream;
+    uint8_t* skip_mask;
+    float* margin;
+};
+
+// Host-side validation shared by the device and host-buffer entry points.
+int validate(const void* q, const void* k, const void* v, void* out, int B, int H, int N, int D,
+             const sparse_attn_params* p, int mode, Resolved* r) {
+    g_last_error[0] = '\0';
+    if (!q || !k || !v || !out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "q, k, v and out must not be NULL");
+    if (mode < SPARSE_ATTN_DENSE || mode > SPARSE_ATTN_DYNAMIC) return fail(SPARSE_ATTN_ERR_MODE, "mode %d not in {0,1,2}", mode);
+    if (B <= 0 || H <= 0 || N <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N must be positive (got %d, %d, %d)", B, H, N);
+    if (static_cast<long long>(B) * H > 65535) return fail(SPARSE_ATTN_ERR_SHAPE, "B*H = %lld exceeds 65535", (long long)B * H);
+    if (N > (1 << 24)) return fail(SPARSE_ATTN_ERR_SHAPE, "N = %d exceeds 2^24", N);
+    if (D != 64 && D != 128) return fail(SPARSE_ATTN_ERR_HEAD_DIM, "D = %d not in {64, 128}", D);
+    if (!p && mode != SPARSE_ATTN_DENSE) return fail(SPARSE_ATTN_ERR_PARAMS, "params must not be NULL in a sparse mode");
+    const int def_tile = (D == 64) ? 64 : 128;
+    r->tile_q = r->tile_k = def_tile;
+    r->scale = 1.0f / std::sqrt(static_cast<float>(D));
+    r->lambda = -INFINITY;
+    r->stream = nullptr;
+    r->skip_mask = nullptr;
+    r->margin = nullptr;
+    if (p) {
+        if (p->struct_size != sizeof(sparse_attn_params))
+            return fail(SPARSE_ATTN_ERR_PARAMS, "params->struct_size = %u, expected %zu", p->struct_size, sizeof(sparse_attn_params));
+        if (std::isnan(p->lambda)) return fail(SPARSE_ATTN_ERR_PARAMS, "lambda is NaN");
+        if (mode == SPARSE_ATTN_FIXED && p->lambda > 0.f)
+            return fail(SPARSE_ATTN_ERR_PARAMS, "lambda = %g > 0 is unsupported in FIXED mode (DESIGN.md R6)", p->lambda);
+        if (!(p->softmax_scale >= 0.f) || std::isinf(p->softmax_scale))
+            return fail(SPARSE_ATTN_ERR_PARAMS, "softmax_scale must be finite and >= 0 (0 = 1/sqrt(D))");
+        const int tq = p->tile_q ? p->tile_q : def_tile;
+        const int tk = p->tile_k ? p->tile_k : tq;
+        if (tq != def_tile || tk != def_tile)
+            return fail(SPARSE_ATTN_ERR_TILE, "decision tile %dx%d unsupported for D = %d (supported: %dx%d)", tq, tk, D, def_tile, def_tile);
+        if (p->softmax_scale > 0.f) r->scale = p->softmax_scale;
+        r->lambda = p->lambda;
+        r->stream = static_cast<cudaStream_t>(p->stream);
+        r->skip_mask = p->skip_mask_out;
+        r->margin = p->margin_out;
+    }
+    return 0;
+}
+
+int check_device() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(SPARSE_ATTN_ERR_DEVICE, "no CUDA device available (this library has no CPU fallback)");
+    }
+    int major = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) {
+        cudaGetLastError();
+        return fail(SPARSE_ATTN_ERR_DEVICE, "device %d has compute capability major %d; sm_100 (B200) is required", dev, major);
+    }
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, float* lse, int B, int H, int N, int D,
+                    const sparse_attn_params* params, int mode, int64_t* stats_out) {
+    Resolved r;
+    int rc = validate(q, k, v, out, B, H, N, D, params, mode, &r);
+    if (rc) return rc;
+    const uintptr_t align_or = reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(k) |
+                               reinterpret_cast<uintptr_t>(v) | reinterpret_cast<uintptr_t>(out);
+    if (align_or & 15u) return fail(SPARSE_ATTN_ERR_ALIGNMENT, "q, k, v and out must be 16-byte aligned");
+    if ((rc = check_device())) return rc;
+
+    EncodeTiledFn enc = nullptr;
+    if ((rc = get_encode_fn(&enc))) return rc;
+    const int BH = B * H;
+    CUtensorMap tq, tk, tv;
+    if ((rc = make_tmap(enc, &tq, q, BH, N, D, 128))) return rc;
+    if ((rc = make_tmap(enc, &tk, k, BH, N, D, r.tile_k))) return rc;
+    if ((rc = make_tmap(enc, &tv, v, BH, N, D, r.tile_k))) return rc;
+
+    dsa::FwdArgs a;
+    a.out = static_cast<__nv_bfloat16*>(out);
+    a.lse = lse;
+    a.stats = reinterpret_cast<unsigned long long*>(stats_out);
+    a.skip_mask = r.skip_mask;
+    a.margin = r.margin;
+    a.N = N;
+    a.T_r = (N + r.tile_q - 1) / r.tile_q;
+    a.T_c = (N + r.tile_k - 1) / r.tile_k;
+    a.n_mma_tiles = (N + 127) / 128;
+    a.mode = mode;
+    a.scale_log2 = r.scale * dsa::kLog2e;
+    a.lambda_log2 = r.lambda * dsa::kLog2e;
+
+    if (stats_out) CUDA_TRY(cudaMemsetAsync(stats_out, 0, sizeof(int64_t) * 2 * BH, r.stream));
+    if (D == 128) return launch<128, 128, 1, 4>(tq, tk, tv, a, BH, r.stream);
+    return launch<64, 64, 2, 4>(tq, tk, tv, a, BH, r.stream);
+}
+
+int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse, int B, int H, int N, int D,
+                         const sparse_attn_params* params, int mode, int64_t* stats_out) {
+    Resolved r;
+    int rc = validate(q, k, v, out, B, H, N, D, params, mode, &r);
+    if (rc) return rc;
+    if ((rc = check_device())) return rc;
+    const size_t n_elem = static_cast<size_t>(B) * H * N * D;
+    const size_t BH = static_cast<size_t>(B) * H;
+    const size_t T_r = (N + r.tile_q - 1) / r.tile_q, T_c = (N + r.tile_k - 1) / r.tile_k;
+    void *dq = nullptr, *dk = nullptr, *dv = nullptr, *dout = nullptr;
+    float *dlse = nullptr, *dmargin = nullptr;
+    int64_t* dstats = nullptr;
+    uint8_t* dmask = nullptr;
+    cudaStream_t st = r.stream;
+    auto cleanup = [&]() {
+        cudaFree(dq); cudaFree(dk); cudaFree(dv); cudaFree(dout); cudaFree(dlse); cudaFree(dstats);
+        cudaFree(dmask); cudaFree(dmargin);
+    };
+#define HOST_TRY(expr)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t err__ = (expr);                                                                      \
+        if (err__ != cudaSuccess) {                                                                      \
+            cleanup();                                                                                   \
+            return fail(SPARSE_ATTN_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(err__));        \
+        }                                                                                                \
+    } while (0)
+    HOST_TRY(cudaMalloc(&dq, n_elem * 2));
+    HOST_TRY(cudaMalloc(&dk, n_elem * 2));
+    HOST_TRY(cudaMalloc(&dv, n_elem * 2));
+    HOST_TRY(cudaMalloc(&dout, n_elem * 2));
+    if (lse) HOST_TRY(cudaMalloc(&dlse, BH * N * sizeof(float)));
+    if (stats_out) HOST_TRY(cudaMalloc(&dstats, BH * 2 * sizeof(int64_t)));
+    if (r.skip_mask) HOST_TRY(cudaMalloc(&dmask, BH * T_r * T_c));
+    if (r.margin) HOST_TRY(cudaMalloc(&dmargin, BH * T_r * T_c * sizeof(float)));
+    HOST_TRY(cudaMemcpyAsync(dq, q, n_elem * 2, cudaMemcpyHostToDevice, st));
+    HOST_TRY(cudaMemcpyAsync(dk, k, n_elem * 2, cudaMemcpyHostToDevice, st));
+    HOST_TRY(cudaMemcpyAsync(dv, v, n_elem * 2, cudaMemcpyHostToDevice, st));
+    sparse_attn_params dp;
+    std::memset(&dp, 0, sizeof dp);
+    if (params) dp = *params;
+    dp.struct_size = sizeof dp;
+    if (!params) dp.lambda = -INFINITY;
+    dp.skip_mask_out = dmask;
+    dp.margin_out = dmargin;
+    rc = sparse_attn_fwd(dq, dk, dv, dout, dlse, B, H, N, D, &dp, mode, dstats);
+    if (rc) { cleanup(); return rc; }
+    HOST_TRY(cudaMemcpyAsync(out, dout, n_elem * 2, cudaMemcpyDeviceToHost, st));
+    if (lse) HOST_TRY(cudaMemcpyAsync(lse, dlse, BH * N * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (stats_out) HOST_TRY(cudaMemcpyAsync(stats_out, dstats, BH * 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    if (r.skip_mask) HOST_TRY(cudaMemcpyAsync(r.skip_mask, dmask, BH * T_r * T_c, cudaMemcpyDeviceToHost, st));
+    if (r.margin) HOST_TRY(cudaMemcpyAsync(r.margin, dmargin, BH * T_r * T_c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    HOST_TRY(cudaStreamSynchronize(st));
+    cleanup();
+#undef HOST_TRY
+    return 0;
+}
+
+double sparse_attn_lambda_from_recall(double recall, int N) { return std::log((1.0 - recall) / N); }
+
+double sparse_attn_lambda_from_preal(double p_real, int tile_k, int N) {
+    return std::log(p_real) + std::log(static_cast<double>(tile_k) / N);
+}
+
+const char* sparse_attn_status_string(int status) {
+    switch (status) {
+        case SPARSE_ATTN_OK: return "ok";
+        case SPARSE_ATTN_ERR_NULL_POINTER: return "required pointer is NULL";
+        case SPARSE_ATTN_ERR_SHAPE: return "bad shape";
+        case SPARSE_ATTN_ERR_HEAD_DIM: return "unsupported head dim";
+        case SPARSE_ATTN_ERR_TILE: return "unsupported decision tile";
+        case SPARSE_ATTN_ERR_MODE: return "bad mode";
+        case SPARSE_ATTN_ERR_PARAMS: return "bad params";
+        case SPARSE_ATTN_ERR_ALIGNMENT: return "misaligned pointer";
+        case SPARSE_ATTN_ERR_DEVICE: return "no sm_100 device";
+        case SPARSE_ATTN_ERR_CUDA: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+const char* sparse_attn_last_error(void) { return g_last_error; }
+
+int sparse_attn_version(void) { return SPARSE_ATTN_VERSION; }
+
+int64_t sparse_attn_launch_count(void) { return g_launches.load(); }
+
+}  // extern "C"
