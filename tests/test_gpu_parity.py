@@ -1,0 +1,215 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Run with `-m gpu` on a B200.  Tolerances are BASELINE.json's (tests/parity_utils.py).
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import MODE_DENSE, MODE_DYNAMIC, MODE_FIXED
+from workloads import CONFIGS, bf16_bits_to_f64, f32_to_bf16_bits, make_head, make_qkv
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def parity():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    import parity_utils
+    return parity_utils
+
+
+def _assert_ok(rep, what):
+    print(f"[parity] {what}: tiles={rep.tiles_checked} decisions={rep.decisions_checked} "
+          f"disagree={rep.disagreements} near-margin-first={rep.near_margin_disagreements} "
+          f"diverged_qtiles={rep.diverged_qtiles} out max-abs={rep.max_abs:.3e} mean-abs={rep.mean_abs:.3e} "
+          f"lse max-abs={rep.max_lse_abs:.3e} margin max-abs={rep.max_margin_abs:.3e}")
+    assert rep.ok(), "\n".join(rep.failures[:10])
+
+
+# ------------------------------------------------------------------ config 0 in full (and its aligned variant)
+CFG0_LAMBDAS = [oracle.lambda_from_recall(r, 1024) for r in (0.90, 0.95, 0.99)] + [-1.0, -2.0, -3.0, -4.0, -6.0]
+
+
+@pytest.mark.parametrize("name", ["cfg0", "cfg0_aligned"])
+def test_cfg0_full_all_modes(parity, seed, name):
+    cfg = CONFIGS[name]
+    q, k, v = make_qkv(cfg, seed)
+    settings = [(MODE_DENSE, -math.inf)] + [(m, lam) for m in (MODE_FIXED, MODE_DYNAMIC) for lam in CFG0_LAMBDAS]
+    total_skipped = 0
+    for mode, lam in settings:
+        gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=cfg.tile)
+        parity.check_stats(gpu, cfg.N, cfg.tile)
+        rep = parity.ParityReport()
+        for h in range(cfg.H):
+            parity.compare_head(gpu, h, q[0, h], k[0, h], v[0, h], tile=cfg.tile, mode=mode, lam=lam, report=rep)
+        _assert_ok(rep, f"{name} mode={mode} lambda={lam:.3f} sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.3f}")
+        if mode == MODE_DENSE:
+            assert gpu.stats[:, 1].sum() == 0
+        total_skipped += int(gpu.stats[:, 1].sum())
+    assert total_skipped > 0       # the skip path really ran
+
+
+# ------------------------------------------------------------------ ragged shapes, several tiles, both head dims
+@pytest.mark.parametrize("B,H,N,D", [(1, 2, 1000, 64), (2, 1, 1000, 128), (1, 1, 40, 64), (1, 1, 129, 128),
+                                     (1, 1, 1, 128), (1, 3, 2125, 128), (1, 1, 64, 64), (1, 1, 193, 64)])
+def test_ragged_random_inputs(parity, seed, B, H, N, D):
+    tile = 64 if D == 64 else 128
+    rng = np.random.default_rng([seed, B, H, N, D])
+    q = f32_to_bf16_bits(rng.standard_normal((B, H, N, D)).astype(np.float32) * 1.8)
+    k = f32_to_bf16_bits(rng.standard_normal((B, H, N, D)).astype(np.float32) * 1.8)
+    v = f32_to_bf16_bits(rng.standard_normal((B, H, N, D)).astype(np.float32))
+    for mode, lam in [(MODE_DENSE, 0.0), (MODE_DYNAMIC, -2.0), (MODE_DYNAMIC, -4.0), (MODE_FIXED, -1.0),
+                      (MODE_FIXED, -3.0), (MODE_DYNAMIC, -math.inf)]:
+        gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=tile)
+        parity.check_stats(gpu, N, tile)
+        rep = parity.ParityReport()
+        for b in range(B):
+            for h in range(H):
+                parity.compare_head(gpu, b * H + h, q[b, h], k[b, h], v[b, h], tile=tile, mode=mode, lam=lam,
+                                    report=rep)
+        _assert_ok(rep, f"ragged B{B} H{H} N{N} D{D} mode={mode} lambda={lam}")
+
+
+def test_softmax_scale_override(parity, seed):
+    rng = np.random.default_rng([seed, 31])
+    q, k, v = (f32_to_bf16_bits(rng.standard_normal((1, 1, 300, 128)).astype(np.float32)) for _ in range(3))
+    gpu = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=-3.0, tile=128, scale=0.2)
+    rep = parity.compare_head(gpu, 0, q[0, 0], k[0, 0], v[0, 0], tile=128, mode=MODE_DYNAMIC, lam=-3.0, scale=0.2)
+    _assert_ok(rep, "scale override")
+
+
+# ------------------------------------------------------------------ closed forms, decisions bit-exact
+def _uniform_inputs(N, D, seed):
+    rng = np.random.default_rng(seed)
+    q = np.zeros((1, 1, N, D), dtype=np.uint16)
+    k = f32_to_bf16_bits(rng.standard_normal((1, 1, N, D)).astype(np.float32))
+    v = f32_to_bf16_bits(rng.standard_normal((1, 1, N, D)).astype(np.float32))
+    return q, k, v
+
+
+@pytest.mark.parametrize("D,tile,N,lam", [(64, 64, 1024, -6.0), (64, 64, 1024, -5.0), (64, 64, 1024, -7.5),
+                                          (128, 128, 2048, -6.0), (128, 128, 2000, -7.0)])
+def test_uniform_closed_form_on_gpu(parity, D, tile, N, lam):
+    """P7 on the GPU: all logits equal -> DYNAMIC keeps exactly k* leading tiles, FIXED skips nothing."""
+    T = -(-N // tile)
+    kept = min(T, int(math.floor(math.exp(-lam) / tile)) + 1)
+    q, k, v = _uniform_inputs(N, D, 3)
+    gpu = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=lam, tile=tile)
+    expect = np.zeros((T, T), dtype=np.uint8)
+    expect[:, kept:] = 1
+    np.testing.assert_array_equal(gpu.skip[0], expect)
+    assert gpu.stats[0].tolist() == [T * kept, T * (T - kept)]
+    vv = bf16_bits_to_f64(v[0, 0])
+    np.testing.assert_allclose(gpu.out[0], np.broadcast_to(vv[:min(N, kept * tile)].mean(axis=0), (N, D)),
+                               atol=parity.OUT_MAX_ABS)
+    np.testing.assert_allclose(gpu.lse[0], math.log(min(N, kept * tile)), atol=parity.LSE_ABS)
+    fix = parity.run_gpu(q, k, v, mode=MODE_FIXED, lam=lam, tile=tile)
+    assert fix.stats[0].tolist() == [T * T, 0]
+
+
+@pytest.mark.parametrize("winner_last", [False, True])
+def test_winner_closed_forms_on_gpu(parity, winner_last):
+    """P8 / P9 on the GPU (D = 128, 128 x 128 tiles)."""
+    N, D, tile, lam, W = 2048, 128, 128, -6.0, 8.0
+    T = N // tile
+    a = math.sqrt(W * math.sqrt(D))
+    a = float(bf16_bits_to_f64(f32_to_bf16_bits(np.float32([a])))[0])
+    Wb = a * a / math.sqrt(D)
+    qf = np.zeros((1, 1, N, D), dtype=np.float32)
+    kf = np.zeros((1, 1, N, D), dtype=np.float32)
+    qf[..., 0] = a
+    kf[0, 0, N - 3 if winner_last else 5, 0] = a
+    v = f32_to_bf16_bits(np.random.default_rng(4).standard_normal((1, 1, N, D)).astype(np.float32))
+    q, k = f32_to_bf16_bits(qf), f32_to_bf16_bits(kf)
+    dyn = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=lam, tile=tile)
+    fix = parity.run_gpu(q, k, v, mode=MODE_FIXED, lam=lam, tile=tile)
+    expect = np.zeros((T, T), dtype=np.uint8)
+    if winner_last:
+        kstar = int(math.floor(math.exp(-lam) / tile)) + 1
+        expect[:, kstar:T - 1] = 1
+        np.testing.assert_array_equal(dyn.skip[0], expect)
+        assert fix.stats[0, 1] == 0
+        np.testing.assert_allclose(dyn.lse[0], math.log(kstar * tile + math.exp(Wb) + tile - 1), atol=parity.LSE_ABS)
+    else:
+        expect[:, 1:] = 1
+        np.testing.assert_array_equal(dyn.skip[0], expect)
+        np.testing.assert_array_equal(fix.skip[0], expect)
+        np.testing.assert_allclose(dyn.lse[0], math.log(math.exp(Wb) + tile - 1), atol=parity.LSE_ABS)
+
+
+# ------------------------------------------------------------------ full-size configs, oracle on sampled Q tiles
+def _sample_qtiles(T, rng, n_random):
+    return sorted(set([0, T - 1] + [int(x) for x in rng.choice(np.arange(1, T - 1), size=n_random, replace=False)]))
+
+
+@pytest.mark.parametrize("name,lam_dyn,lam_fix", [("cfg1", -3.0, -1.0), ("cfg1_aligned", -6.0, -6.0)])
+def test_cfg1_full_size_sampled_tiles(parity, seed, name, lam_dyn, lam_fix):
+    """Config 1 (B=1, H=24, N=32760, D=128) in the launch configuration bench.py times; the oracle checks
+    the first, the last (ragged) and random Q tiles of 3 heads against all 256 K tiles."""
+    cfg = CONFIGS[name]
+    q, k, v = make_qkv(cfg, seed)
+    rng = np.random.default_rng([seed, 1234])
+    heads = [0, 11, 23]
+    for mode, lam in [(MODE_DENSE, -math.inf), (MODE_DYNAMIC, lam_dyn), (MODE_FIXED, lam_fix)]:
+        gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=cfg.tile)
+        parity.check_stats(gpu, cfg.N, cfg.tile)
+        rep = parity.ParityReport()
+        for h in heads:
+            qt = _sample_qtiles(256, rng, 2)
+            parity.compare_head(gpu, h, q[0, h], k[0, h], v[0, h], tile=cfg.tile, mode=mode, lam=lam, qtiles=qt,
+                                report=rep)
+        _assert_ok(rep, f"{name} mode={mode} lambda={lam} sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.4f}")
+
+
+def test_cfg3_shape_sampled_tiles(parity, seed):
+    """Config 3's N = 75600 (591 tiles: odd tile count, 80-row ragged tail) on 2 heads of the aligned variant."""
+    cfg = CONFIGS["cfg3_aligned"]
+    q, k, v = make_qkv(cfg, seed, heads=[3, 17])
+    rng = np.random.default_rng([seed, 4321])
+    for mode, lam in [(MODE_DYNAMIC, -6.0), (MODE_FIXED, -6.0)]:
+        gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=cfg.tile)
+        parity.check_stats(gpu, cfg.N, cfg.tile)
+        rep = parity.ParityReport()
+        for h in range(2):
+            qt = [0, 590] + [int(x) for x in rng.choice(np.arange(1, 590), size=1)]
+            parity.compare_head(gpu, h, q[0, h], k[0, h], v[0, h], tile=cfg.tile, mode=mode, lam=lam, qtiles=qt,
+                                report=rep)
+        _assert_ok(rep, f"cfg3_aligned mode={mode} lambda={lam} sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.4f}")
+
+
+# ------------------------------------------------------------------ invariants that hold at any size
+def test_dynamic_superset_of_fixed_and_recall_on_gpu(parity, seed):
+    """P6 and P3 evaluated from GPU outputs alone on full config-1-shaped heads (aligned variant)."""
+    cfg = CONFIGS["cfg1_aligned"]
+    q, k, v = make_qkv(cfg, seed, heads=[2, 9])
+    lam = -8.0
+    dense = parity.run_gpu(q, k, v, mode=MODE_DENSE, tile=cfg.tile, debug=False)
+    dyn = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=lam, tile=cfg.tile)
+    fix = parity.run_gpu(q, k, v, mode=MODE_FIXED, lam=lam, tile=cfg.tile)
+    # P6 holds exactly in exact arithmetic; on the GPU allow disagreement only at near-margin tiles
+    viol = (fix.skip == 1) & (dyn.skip == 0)
+    assert np.all(np.abs(dyn.margin[viol]) <= parity.MARGIN_TOL)
+    assert dyn.stats[:, 1].sum() >= fix.stats[:, 1].sum() - viol.sum()
+    for res in (dyn, fix):
+        recall = np.exp(res.lse.astype(np.float64) - dense.lse.astype(np.float64))
+        skipped_cols = np.repeat(res.skip.sum(axis=2) * cfg.tile, cfg.tile, axis=1)[:, :cfg.N]
+        assert np.all(1.0 - recall < skipped_cols * math.exp(lam) + 5e-3)   # P3 (+ fp32 lse rounding)
+
+
+def test_host_buffer_entry_point(parity, seed):
+    import paper_2606_16317_b200 as sa
+    cfg = CONFIGS["cfg0"]
+    q, k, v = make_qkv(cfg, seed)
+    out = np.zeros_like(q)
+    lse = np.zeros((1, cfg.H, cfg.N), dtype=np.float32)
+    stats = np.zeros((1, cfg.H, 2), dtype=np.int64)
+    p = sa.make_params(lam=-2.0)
+    sa.sparse_attn_fwd_host(q, k, v, out, lse, 1, cfg.H, cfg.N, cfg.D, p, MODE_DYNAMIC, stats)
+    dev = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=-2.0, tile=cfg.tile)
+    np.testing.assert_array_equal(bf16_bits_to_f64(out).reshape(cfg.H, cfg.N, cfg.D), dev.out)
+    np.testing.assert_array_equal(stats.reshape(cfg.H, 2), dev.stats)
