@@ -1,0 +1,357 @@
+#!/usr/bin/env python
+"""bench.py -- times the tile-skipping attention forward on synthetic Wan-2.2-shaped inputs.
+
+One "step" = one sparse_attn_fwd call (the whole hot path) over one
+batch of BASELINE.json config 1 (B=1, H=24, N=32760, D=128, 128x128 tiles) in DYNAMIC mode at the
+paper's Eq. 7 threshold (P_real = 1.5).  The same kernel's DENSE and FIXED modes are timed beside
+it, on the contract ("literal") generator and on the supplementary aligned variant.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Prints ONE JSON line on rank 0.  N > 1 (under torchrun): every rank runs its own config-1 batch
+(heads are independent units: no data-path collective, weak scaling), stats are all-gathered.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from workloads import CONFIGS, make_qkv  # noqa: E402
+
+METRIC = "attention ms & effective TFLOP/s vs dense mode at Wan-2.2 shapes; sparsity %; % tensor peak"
+P_REAL = 1.5            # Eq. 7 "transition region" constant
+FALLBACK_TFLOPS = 1590.0
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["bf16_tflops"]), float(p.get("bf16_tflops_sustained", p["bf16_tflops"])), "measured"
+    return FALLBACK_TFLOPS, 1400.0, "fallback"
+
+
+def dense_flop(BH, N, D):
+    return 4.0 * BH * N * N * D
+
+
+def executed_flop(BH, N, D, tile, stats):
+    """QK^T for every tile + P V for executed tiles; ragged tiles counted as full
+    in the P V term (error < 1/T_c)."""
+    qk = 2.0 * BH * N * N * D
+    T = -(-N // tile)
+    frac_exec = float(stats[..., 0].sum()) / float(BH * T * T)
+    return qk + 2.0 * BH * N * N * D * frac_exec
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.samples, self._stop, self.index = [], threading.Event(), index
+        self._t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.samples.append([s.strip() for s in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        sm = [float(s[0]) for s in self.samples if len(s) >= 7 and s[0].replace(".", "").isdigit()]
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            if len(s) >= 7:
+                for n, val in zip(names, s[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(n)
+        mx = [float(s[1]) for s in self.samples if len(s) >= 7 and s[1].replace(".", "").isdigit()]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------- oracle arm
+def oracle_sample_time(cfg, seed, lam, mode, head=0, reps=1):
+    """Time the oracle, as it stands, on a bounded sample: up to 16 x (host threads) Q tiles of one head
+    (for config 1 on a 16-core box that is one full head, all 256 Q tiles)."""
+    import oracle
+    q, k, v = make_qkv(cfg, seed, heads=[head])
+    cores = oracle.max_threads()
+    T = -(-cfg.N // cfg.tile)
+    n_tiles = min(T, 16 * cores)
+    qt = [int(x) for x in np.linspace(0, T - 1, n_tiles).round()]
+    qt = sorted(set(qt))
+    times = []
+    for _ in range(reps):
+        t0 = time.perf_counter()
+        oracle.run_head(q[0, 0], k[0, 0], v[0, 0], tile=cfg.tile, lam=lam, mode=mode, qtiles=qt)
+        times.append(time.perf_counter() - t0)
+    rows = sum(min(cfg.tile, cfg.N - i * cfg.tile) for i in qt)
+    flop = 4.0 * rows * cfg.N * cfg.D                    # dense-equivalent FLOP of the sampled Q tiles
+    return {"seconds": times, "flop": flop, "cores": cores, "n_qtiles": len(qt),
+            "sample": f"{len(qt)} of {T} Q tiles (evenly spaced, incl. first and ragged last) of head {head}, "
+                      f"all {T} K tiles, mode {mode}, lambda {lam:.3f}"}
+
+
+def run_reference(args, cfg, lam):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    res = oracle_sample_time(cfg, args.seed, lam, 2, reps=args.warmup + args.steps)
+    secs = res["seconds"][args.warmup:]
+    mean_s = float(np.mean(secs))
+    val = res["flop"] / mean_s / 1e12
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "TFLOP/s (dense-equivalent, effective)",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": mean_s * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "mode": "dynamic", "lambda": lam, "step": res["sample"]},
+        "cpu_baseline": {"value": val, "unit": "TFLOP/s (dense-equivalent, effective)", "cores": res["cores"],
+                         "kind": "oracle", "sample": res["sample"]},
+        "e2e": {"value": val, "unit": "TFLOP/s (dense-equivalent, effective)", "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg):
+    return (f"BASELINE.json configs[1] ({cfg.name}): B={cfg.B} H={cfg.H} N={cfg.N} (grid {cfg.grid}) D={cfg.D}, "
+            f"{cfg.tile}x{cfg.tile} tiles, generator sigma={cfg.sigma} a={cfg.noise_a} tau={cfg.tau}")
+
+
+# ---------------------------------------------------------------------------------------------- GPU arm
+def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier):
+    """Returns (total_ms over `steps` calls, per-call ms list, stats [B,H,2])."""
+    q, k, v, out, lse, stats = bufs
+    stream = torch.cuda.current_stream()
+    p = sa.make_params(lam=lam, stream=stream.cuda_stream)
+    for _ in range(warmup):
+        sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p, mode, stats)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    barrier()
+    torch.cuda.synchronize()
+    evs[0].record(stream)
+    for i in range(steps):
+        sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p, mode, stats)
+        evs[i + 1].record(stream)
+    torch.cuda.synchronize()
+    barrier()
+    per = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
+    return evs[0].elapsed_time(evs[-1]), per, stats.cpu().numpy().copy()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--seed", type=int, default=20261104)
+    ap.add_argument("--config", default="cfg1")
+    ap.add_argument("--no-aligned", action="store_true", help="skip the supplementary aligned workload")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--modes", default="dense,fixed,dynamic", help="subset of modes to time (profiling runs)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    cfg = CONFIGS[args.config]
+    lam = math.log(P_REAL) + math.log(cfg.tile / cfg.N)        # Eq. 7
+    if args.impl == "reference":
+        run_reference(args, cfg, lam)
+        return
+
+    import torch
+    import paper_2606_16317_b200 as sa   # raises if the CUDA extension is missing: no fallback
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (B200); there is no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    tb, ts, peak_kind = measured_peaks()
+    BH = cfg.B * cfg.H
+
+    def to_dev(bits):
+        return torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+
+    results = {}
+    variants = [args.config] + ([] if args.no_aligned or args.config + "_aligned" not in CONFIGS
+                                else [args.config + "_aligned"])
+    clocks = None
+    head_total_ms = None
+    launches0 = sa.launch_count()
+    headline_launches = 0
+    for vi, name in enumerate(variants):
+        vcfg = CONFIGS[name]
+        # weak scaling: every rank draws its own batch (different seed), same shape
+        qb, kb, vb = make_qkv(vcfg, args.seed + 1000 * rank)
+        q, k, v = to_dev(qb), to_dev(kb), to_dev(vb)
+        out = torch.empty_like(q)
+        lse = torch.empty((cfg.B, cfg.H, cfg.N), device="cuda", dtype=torch.float32)
+        stats = torch.zeros((cfg.B, cfg.H, 2), device="cuda", dtype=torch.int64)
+        bufs = (q, k, v, out, lse, stats)
+        res = {}
+        for mname, mode, mlam in (("dense", sa.MODE_DENSE, -math.inf), ("fixed", sa.MODE_FIXED, lam),
+                                  ("dynamic", sa.MODE_DYNAMIC, lam)):
+            if mname not in args.modes.split(","):
+                continue
+            headline = (vi == 0 and mname == "dynamic")
+            if headline:
+                l0 = sa.launch_count()
+                with ClockSampler(local_rank) as cs:
+                    total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier)
+                headline_launches = sa.launch_count() - l0 - args.warmup
+                clocks = cs.summary()
+                head_total_ms = total
+            else:
+                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier)
+            if dist is not None:
+                t = torch.tensor([total], device="cuda")
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                total = float(t.item())
+                gathered = [torch.zeros_like(stats) for _ in range(world)]
+                dist.all_gather(gathered, torch.from_numpy(st).cuda())     # [world][B,H,2]: per-head counts
+                st_all = torch.stack(gathered).cpu().numpy()
+            else:
+                st_all = st[None]
+            ms = total / args.steps
+            ex = executed_flop(BH * world, cfg.N, cfg.D, cfg.tile, st_all)
+            res[mname] = {
+                "ms": ms, "ms_min": float(np.min(per)), "ms_median": float(np.median(per)),
+                "sparsity": float(st_all[..., 1].sum() / st_all.sum()),
+                "effective_tflops": dense_flop(BH * world, cfg.N, cfg.D) / (ms * 1e-3) / 1e12,
+                "executed_tflops": ex / (ms * 1e-3) / 1e12,
+                "kernel_ms_avg_rank0": float(np.mean(per)),
+                "executed_flop_per_launch_rank0": executed_flop(BH, cfg.N, cfg.D, cfg.tile, st[None]),
+            }
+        for mname in ("fixed", "dynamic"):
+            if mname not in res or "dense" not in res:
+                continue
+            res[mname]["speedup_vs_dense"] = res["dense"]["ms"] / res[mname]["ms"]
+            res[mname]["mma_bound_model"] = 1.0 / (1.0 - res[mname]["sparsity"] / 2.0)
+        results[name] = res
+        if vi == 0:
+            keep_bufs = (qb, kb, vb)
+        del q, k, v, out, lse, stats, bufs
+        torch.cuda.empty_cache()
+
+    # ------------------------------------------------------------------ end-to-end through the host-buffer C entry point
+    qb, kb, vb = keep_bufs
+    hq, hk, hv = (torch.from_numpy(x.view(np.int16)).pin_memory() for x in (qb, kb, vb))
+    hout = torch.empty_like(hq).pin_memory()
+    hlse = torch.empty((cfg.B, cfg.H, cfg.N), dtype=torch.float32).pin_memory()
+    hstats = torch.zeros((cfg.B, cfg.H, 2), dtype=torch.int64).pin_memory()
+    p = sa.make_params(lam=lam, stream=torch.cuda.current_stream().cuda_stream)
+    e2e_steps = max(3, min(args.steps, 5))
+    sa.sparse_attn_fwd_host(hq, hk, hv, hout, hlse, cfg.B, cfg.H, cfg.N, cfg.D, p, sa.MODE_DYNAMIC, hstats)
+    barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sa.sparse_attn_fwd_host(hq, hk, hv, hout, hlse, cfg.B, cfg.H, cfg.N, cfg.D, p, sa.MODE_DYNAMIC, hstats)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    barrier()
+    h2d = 3 * hq.numel() * 2
+    d2h = hout.numel() * 2 + hlse.numel() * 4 + hstats.numel() * 8
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ------------------------------------------------------------------ CPU baseline: the oracle as it stands
+    cpu_baseline = None
+    if not args.no_cpu_baseline and world == 1:
+        r = oracle_sample_time(cfg, args.seed, lam, 2)
+        cpu_baseline = {"value": r["flop"] / r["seconds"][0] / 1e12, "unit": "TFLOP/s (dense-equivalent, effective)",
+                        "cores": r["cores"], "kind": "oracle", "sample": r["sample"], "seconds": r["seconds"][0],
+                        "extrapolated_full_config_seconds": r["seconds"][0] * dense_flop(BH, cfg.N, cfg.D) / r["flop"]}
+
+    if set(args.modes.split(",")) != {"dense", "fixed", "dynamic"}:      # profiling run: raw numbers only
+        print(json.dumps({"partial": True, "modes": results, "lambda": lam}), flush=True)
+        return
+    main_res = results[args.config]["dynamic"]
+    dense_res = results[args.config]["dense"]
+    # roofline of the dominant (only) kernel, in the mode with the most executed work per launch: DENSE
+    ach = dense_res["executed_flop_per_launch_rank0"] / (dense_res["kernel_ms_avg_rank0"] * 1e-3) / 1e12
+    ach_dyn = main_res["executed_flop_per_launch_rank0"] / (main_res["kernel_ms_avg_rank0"] * 1e-3) / 1e12
+    line = {
+        "metric": METRIC,
+        "value": main_res["effective_tflops"],
+        "unit": "TFLOP/s (dense-equivalent attention FLOP / time, DYNAMIC mode)",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": head_total_ms / args.steps if world == 1 else main_res["ms"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "mode": "dynamic", "lambda": lam,
+                   "lambda_rule": f"Eq. 7, P_real={P_REAL}", "l2": "q+k+v+out = 805 MB per step > 126 MB L2, no flush",
+                   "parallelism": f"heads sharded, {world} rank(s), no data-path collective"},
+        "sparsity_pct": 100.0 * main_res["sparsity"],
+        "speedup_vs_dense": main_res["speedup_vs_dense"],
+        "pct_tensor_peak_executed": {"dense": 100.0 * ach / tb, "dynamic": 100.0 * ach_dyn / tb,
+                                     "of": f"{tb} TFLOP/s ({peak_kind} burst)"},
+        "modes": results,
+        "roofline": {"bound": "tensor", "achieved": ach, "peak": tb, "unit": "TFLOP/s", "frac": ach / tb,
+                     "traffic": None, "kernel": "sparse_attn_fwd_kernel<128,128,1,*> DENSE mode",
+                     "peak_kind": f"{peak_kind} bf16 burst; sustained {ts}", "frac_sustained": ach / ts,
+                     "frac_dynamic_mode": ach_dyn / tb,
+                     "flop_per_launch": dense_res["executed_flop_per_launch_rank0"],
+                     "launch_ms": dense_res["kernel_ms_avg_rank0"]},
+        "cpu_baseline": cpu_baseline,
+        "e2e": {"value": dense_flop(BH * world, cfg.N, cfg.D) / e2e_s / 1e12,
+                "unit": "TFLOP/s (dense-equivalent, host buffers, H2D + kernel + D2H)",
+                "ms_per_step": e2e_s * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": headline_launches,
+        "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

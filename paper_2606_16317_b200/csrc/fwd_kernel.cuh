@@ -8,6 +8,7 @@
 //   warps 4-7   softmax warpgroup of slot 1
 //   warp  8     TMA producer: Q once, then K_0, V_0, K_1, V_1, ... through an NSTAGE mbarrier ring
 //   warp  9     tcgen05.mma issuer (one elected thread) and TMEM owner
+//   warps 10-11 idle (they complete the third warpgroup so that setmaxnreg can hand its registers over)
 // TMEM (512 columns): S_0 | S_1 (fp32, BC columns each; P_X, bf16x2, aliases the first BC/2 columns of S_X)
 //                     O_0 | O_1 (fp32, D columns each).
 // Per slot X and K tile j:  S_X = Q_X K_j^T (always)  ->  softmax warpgroup: row max, skip predicate,
@@ -24,9 +25,13 @@ namespace dsa {
 
 enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2 };
 
-constexpr int kNumThreads = 320;
+constexpr int kNumThreads = 384;      // 3 warpgroups: softmax 0, softmax 1, {producer, MMA, 2 idle warps}
 constexpr int kProducerWarp = 8;
 constexpr int kMmaWarp = 9;
+// setmaxnreg: the kernel launches with 168 registers/thread (65536 / 384); the two softmax warpgroups
+// grow to 232 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 40.
+constexpr int kRegsSoftmax = 232;
+constexpr int kRegsOther = 40;
 constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -66,7 +71,9 @@ struct SmemLayout {
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
 };
 
-template <int D, int BC, int G, int NSTAGE>
+// kSparse = false compiles the DENSE mode only (no predicate, no vote); kDebug adds the optional
+// skip_mask_out / margin_out parity outputs.
+template <int D, int BC, int G, int NSTAGE, bool kSparse, bool kDebug>
 __global__ void __launch_bounds__(kNumThreads, 1)
 sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                        const __grid_constant__ CUtensorMap tm_v, const FwdArgs a) {
@@ -132,7 +139,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
 
-    if (warp == kProducerWarp) {
+    if (warp >= 8) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
+        if (warp == kProducerWarp) {
         // ============================================================== TMA producer (a1)
         if (lane == 0) {
             for (int x = 0; x < nX; ++x) {
@@ -154,7 +163,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
         }
         __syncwarp();
-    } else if (warp == kMmaWarp) {
+        } else if (warp == kMmaWarp) {
         // ============================================================== MMA issuer (a2, a6)
         if (lane == 0) {
             auto issue_qk = [&](int x, uint32_t kaddr) {
@@ -200,7 +209,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 for (int x = 0; x < nX; ++x) {
                     mbar_wait(p_ready(x), j & 1);
                     tc_fence_after();
-                    const int keep = keepflag[x * 2 + (j & 1)];
+                    const int keep = kSparse ? keepflag[x * 2 + (j & 1)] : 1;
                     if (keep) {
                         if (!v_waited) { mbar_wait(kv_full(v_stage), v_phase); tc_fence_after(); v_waited = true; }
                         issue_pv(x, kv_smem + v_stage * L::kKVStageBytes, j > 0);
@@ -219,7 +228,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
         }
         __syncwarp();
-    } else if (warp < 4 * nX) {
+        }
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
+        if (warp < 4 * nX) {
         // ============================================================== softmax warpgroups (a3-a5, a7-a9)
         const int x = warp >> 2;
         const int w = warp & 3;
@@ -238,7 +250,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         const int mode = a.mode;
         const float scale_log2 = a.scale_log2;
         const float lambda_log2 = a.lambda_log2;
-        const bool want_margin = a.margin != nullptr;
+        const bool want_margin = kDebug && a.margin != nullptr;
 
         float m_used = -INFINITY;   // stabiliser actually subtracted (log2 domain, may lag the true max)
         float m_true = -INFINITY;   // running max over retained tiles (log2 domain) -- FIXED mode reference
@@ -260,15 +272,20 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 for (int c = 0; c < BC; ++c)
                     if (c >= valid_cols) su[c >> 5][c & 31] = 0xff800000u;
             }
-            float mhat = S_AT(0);
+            float mx0 = S_AT(0), mx1 = S_AT(1), mx2 = S_AT(2), mx3 = S_AT(3);   // 4 independent max chains
 #pragma unroll
-            for (int c = 1; c < BC; ++c) mhat = fmaxf(mhat, S_AT(c));
-            const float mhat2 = mhat * scale_log2;           // tile-local row max, log2 domain (a3)
+            for (int c = 4; c < BC; c += 4) {
+                mx0 = fmaxf(mx0, S_AT(c));
+                mx1 = fmaxf(mx1, S_AT(c + 1));
+                mx2 = fmaxf(mx2, S_AT(c + 2));
+                mx3 = fmaxf(mx3, S_AT(c + 3));
+            }
+            const float mhat2 = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;   // tile-local row max (a3)
 
             // ---- predicate and all-rows vote (a4)
             bool skip_grp = false, keep_any = true;
             float grp_margin = INFINITY;
-            if (mode != kModeDense && j > 0) {
+            if (kSparse && j > 0) {
                 const float ref = (mode == kModeDynamic) ? (m_used + fast_log2(l)) : m_true;
                 const float t2 = mhat2 - ref;                // Eq. 5 in log2 units
                 const bool row_skip = !row_valid || (t2 < lambda_log2);
@@ -300,22 +317,26 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
             if (grp_leader && grp_valid) {                   // a9 + optional parity outputs
                 if (skip_grp) ++n_skip; else ++n_exec;
-                if (a.skip_mask) a.skip_mask[tile_row + j] = skip_grp ? 1 : 0;
-                if (want_margin) a.margin[tile_row + j] = grp_margin;
+                if (kDebug) {
+                    if (a.skip_mask) a.skip_mask[tile_row + j] = skip_grp ? 1 : 0;
+                    if (want_margin) a.margin[tile_row + j] = grp_margin;
+                }
             }
 
-            if (!keep_any) {                                 // a7: skipped -- m, l, O untouched
+            if (kSparse && !keep_any) {                      // a7: skipped -- m, l, O untouched
                 if (r == 0) keepflag[x * 2 + par] = 0;
                 tc_fence_before();
                 mbar_arrive(p_ready(x));
                 continue;
             }
 
-            uint32_t pk[BC / 64][32];
-            if (G == 2 && skip_grp) {
+            if (kSparse && G == 2 && skip_grp) {
                 // this half skipped but its partner half kept: contribute P = 0, statistics untouched
+                uint32_t z[16];
 #pragma unroll
-                for (int c = 0; c < BC / 2; ++c) pk[c >> 5][c & 31] = 0u;
+                for (int i = 0; i < 16; ++i) z[i] = 0u;
+#pragma unroll
+                for (int c = 0; c < BC / 32; ++c) tmem_st_x16(tS + c * 16, z);
             } else {
                 // ---- online softmax update (a5)
                 if (j == 0) {
@@ -338,23 +359,27 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     }
                 }
                 m_true = fmaxf(m_true, mhat2);
-                float rowsum = 0.f;
+                const float neg_m = -m_used;
+                float rs0 = 0.f, rs1 = 0.f;
 #pragma unroll
-                for (int c = 0; c < BC; c += 2) {
-                    const float p0 = fast_exp2(fmaf(S_AT(c), scale_log2, -m_used));
-                    const float p1 = fast_exp2(fmaf(S_AT(c + 1), scale_log2, -m_used));
-                    rowsum += p0 + p1;
-                    pk[c >> 6][(c >> 1) & 31] = pack_bf16x2(p0, p1);
+                for (int c = 0; c < BC / 32; ++c) {          // 32 columns -> 16 packed bf16x2 -> P columns [16c, 16c+16)
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        const float p0 = fast_exp2(fmaf(__uint_as_float(su[c][2 * i]), scale_log2, neg_m));
+                        const float p1 = fast_exp2(fmaf(__uint_as_float(su[c][2 * i + 1]), scale_log2, neg_m));
+                        rs0 += p0;
+                        rs1 += p1;
+                        pk[i] = pack_bf16x2(p0, p1);
+                    }
+                    tmem_st_x16(tS + c * 16, pk);
                 }
-                l += rowsum;
+                l += rs0 + rs1;
             }
-#pragma unroll
-            for (int c = 0; c < BC / 64; ++c)                // P (bf16x2) over the first BC/2 columns of S
-                tmem_st_x32(tS + c * 32, pk[c]);
 #undef S_AT
             tmem_wait_st();
             tc_fence_before();
-            if (r == 0) keepflag[x * 2 + par] = 1;
+            if (kSparse && r == 0) keepflag[x * 2 + par] = 1;
             mbar_arrive(p_ready(x));
         }
 
@@ -385,6 +410,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         if (a.stats && grp_leader && grp_valid) {
             atomicAdd(a.stats + 2 * bh + 0, static_cast<unsigned long long>(n_exec));
             atomicAdd(a.stats + 2 * bh + 1, static_cast<unsigned long long>(n_skip));
+        }
         }
     }
 

@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "fwd_kernel.cuh"
@@ -62,11 +63,11 @@ int make_tmap(EncodeTiledFn enc, CUtensorMap* tm, const void* base, int BH, int 
     return 0;
 }
 
-template <int D, int BC, int G, int NSTAGE>
+template <int D, int BC, int G, int NSTAGE, bool kSparse, bool kDebug>
 int launch(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const dsa::FwdArgs& args, int BH,
            cudaStream_t stream) {
     using L = dsa::SmemLayout<D, BC, NSTAGE>;
-    auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NSTAGE>;
+    auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NSTAGE, kSparse, kDebug>;
     static bool configured = false;
     if (!configured) {
         CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L::kDynamicBytes));
@@ -177,8 +178,18 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     a.lambda_log2 = r.lambda * dsa::kLog2e;
 
     if (stats_out) CUDA_TRY(cudaMemsetAsync(stats_out, 0, sizeof(int64_t) * 2 * BH, r.stream));
-    if (D == 128) return launch<128, 128, 1, 4>(tq, tk, tv, a, BH, r.stream);
-    return launch<64, 64, 2, 4>(tq, tk, tv, a, BH, r.stream);
+    const bool sparse = mode != SPARSE_ATTN_DENSE;
+    const bool debug = r.skip_mask || r.margin;
+    if (D == 128) {
+        if (!sparse && !debug) return launch<128, 128, 1, 4, false, false>(tq, tk, tv, a, BH, r.stream);
+        if (!sparse) return launch<128, 128, 1, 4, false, true>(tq, tk, tv, a, BH, r.stream);
+        if (!debug) return launch<128, 128, 1, 4, true, false>(tq, tk, tv, a, BH, r.stream);
+        return launch<128, 128, 1, 4, true, true>(tq, tk, tv, a, BH, r.stream);
+    }
+    if (!sparse && !debug) return launch<64, 64, 2, 4, false, false>(tq, tk, tv, a, BH, r.stream);
+    if (!sparse) return launch<64, 64, 2, 4, false, true>(tq, tk, tv, a, BH, r.stream);
+    if (!debug) return launch<64, 64, 2, 4, true, false>(tq, tk, tv, a, BH, r.stream);
+    return launch<64, 64, 2, 4, true, true>(tq, tk, tv, a, BH, r.stream);
 }
 
 int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse, int B, int H, int N, int D,
