@@ -14,7 +14,7 @@ from typing import Optional
 MODE_DENSE, MODE_FIXED, MODE_DYNAMIC = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libsparse_attn.so")
+_LIB_PATH = os.environ.get("SPARSE_ATTN_LIB") or os.path.join(_HERE, "libsparse_attn.so")
 _lib = None
 
 # every symbol include/sparse_attn.h declares

@@ -6,9 +6,11 @@
 // CTA = 2 MMA tiles (slots X = 0, 1) of 128 query rows of one (b, h), sharing every K_j / V_j tile:
 //   warps 0-3   softmax warpgroup of slot 0 (thread <-> query row <-> TMEM lane)
 //   warps 4-7   softmax warpgroup of slot 1
-//   warp  8     TMA producer: Q once, then K_0, V_0, K_1, V_1, ... through an NSTAGE mbarrier ring
-//   warp  9     tcgen05.mma issuer (one elected thread) and TMEM owner
-//   warps 10-11 idle (they complete the third warpgroup so that setmaxnreg can hand its registers over)
+//   warp  8     TMA producer for Q (once) and the K ring (runs ahead of the decisions)
+//   warp  9     tcgen05.mma issuer (one elected lane) and TMEM owner
+//   warp  10    TMA producer for the V ring in DENSE mode (in the sparse modes the MMA warp fetches V_j itself,
+//               and only if some slot keeps tile j or tile j-1 needed its V)
+//   warp  11    idle (completes the third warpgroup so that setmaxnreg can hand its registers over)
 // TMEM (512 columns): S_0 | S_1 (fp32, BC columns each; P_X, bf16x2, aliases the first BC/2 columns of S_X)
 //                     O_0 | O_1 (fp32, D columns each).
 // Per slot X and K tile j:  S_X = Q_X K_j^T (always)  ->  softmax warpgroup: row max, skip predicate,
@@ -23,20 +25,39 @@
 
 namespace dsa {
 
+#ifdef DSA_PROF
+#define PROF_DECL(n) unsigned long long prof_acc[n] = {}; long long prof_t = clock64();
+#define PROF_TICK(i) { long long t__ = clock64(); prof_acc[i] += t__ - prof_t; prof_t = t__; }
+#define PROF_FLUSH(base, n, cond) if (a.prof && (cond)) { for (int i__ = 0; i__ < n; ++i__) a.prof[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * 32 + base + i__] = prof_acc[i__]; }
+#define TRACE(slot) if (a.prof && blockIdx.x == 0 && blockIdx.y == 0 && j < 32 && (threadIdx.x & 31) == 0) a.prof[(1 << 20) + (j * 2 + x) * 16 + (slot)] = clock64();
+#else
+#define TRACE(slot)
+#define PROF_DECL(n)
+#define PROF_TICK(i)
+#define PROF_FLUSH(base, n, cond)
+#endif
+
 enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2 };
 
-constexpr int kNumThreads = 384;      // 3 warpgroups: softmax 0, softmax 1, {producer, MMA, 2 idle warps}
-constexpr int kProducerWarp = 8;
+constexpr int kNumThreads = 384;      // 3 warpgroups
+constexpr int kKProducerWarp = 8;
 constexpr int kMmaWarp = 9;
+constexpr int kVProducerWarp = 10;
 // setmaxnreg: the kernel launches with 168 registers/thread (65536 / 384); the two softmax warpgroups
-// grow to 232 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 40.
-constexpr int kRegsSoftmax = 232;
-constexpr int kRegsOther = 40;
+// grow to 224 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 56.
+constexpr int kRegsSoftmax = 224;
+constexpr int kRegsOther = 56;
 constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 // lazy rescale: O and l are only rescaled when the row max grew by more than 2^8 (log2 domain).
 constexpr float kRescaleThreshold = 8.0f;
+// of every 16 (p0, p1) pairs of a 32-column chunk, this many are exponentiated on the FMA pipe (exp2_fma).
+// Measured on B200: the softmax warps are issue-bound, not MUFU-bound, so 0 is fastest.
+#ifndef DSA_EMUL_PAIRS
+#define DSA_EMUL_PAIRS 0
+#endif
+constexpr int kEmulPairs = DSA_EMUL_PAIRS;
 
 struct FwdArgs {
     __nv_bfloat16* out;          // [BH, N, D]
@@ -51,33 +72,39 @@ struct FwdArgs {
     int mode;
     float scale_log2;            // softmax_scale * log2(e)
     float lambda_log2;           // lambda * log2(e)
+#ifdef DSA_PROF
+    unsigned long long* prof;    // [n_cta][32] cycle counters (profiling builds only)
+#endif
 };
 
-template <int D, int BC, int NSTAGE>
+template <int D, int BC, int NK, int NV>
 struct SmemLayout {
     static constexpr int kQSlotBytes = 128 * D * 2;
     static constexpr int kSubQBytes = 128 * 128;        // one 64-column (128 B) sub-tile of Q
     static constexpr int kKVStageBytes = BC * D * 2;
     static constexpr int kSubKVBytes = BC * 128;        // one 64-column sub-tile of K or V
     static constexpr int kQOff = 0;
-    static constexpr int kKVOff = 2 * kQSlotBytes;
-    static constexpr int kBarOff = kKVOff + NSTAGE * kKVStageBytes;
-    // barriers (8 B each): q_full[2], kv_full[NSTAGE], kv_empty[NSTAGE], s_full[2], p_ready[2], o_full[2]
-    static constexpr int kNumBars = 2 + 2 * NSTAGE + 6;
+    static constexpr int kKOff = 2 * kQSlotBytes;
+    static constexpr int kVOff = kKOff + NK * kKVStageBytes;
+    static constexpr int kBarOff = kVOff + NV * kKVStageBytes;
+    // barriers (8 B each): q_full[2] k_full[NK] k_empty[NK] v_full[NV] v_empty[NV]
+    //                      s_full[2] p_half[2] p_ready[2] o_full[2] (2 unused) dec[2]
+    static constexpr int kNumBars = 2 + 2 * NK + 2 * NV + 8 + 2 + 2;
     static constexpr int kMiscOff = kBarOff + 8 * kNumBars;
-    // misc: tmem_ptr (4) | keepflag[2][2] (16) | votes[2][2][4] (64) | wmax[2][2][4] (64)
-    static constexpr int kMiscBytes = 4 + 16 + 64 + 64 + 12;
+    // misc: tmem_ptr (4) | pad (44) | votes[2][2][4] (64) | wmax[2][2][4] (64)
+    static constexpr int kMiscBytes = 16 + 16 + 16 + 64 + 64;
     static constexpr int kTotal = kMiscOff + kMiscBytes;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
+    static_assert(kDynamicBytes <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
 };
 
-// kSparse = false compiles the DENSE mode only (no predicate, no vote); kDebug adds the optional
-// skip_mask_out / margin_out parity outputs.
-template <int D, int BC, int G, int NSTAGE, bool kSparse, bool kDebug>
+// kSparse = false compiles the DENSE mode only (no predicate, no vote, V always fetched);
+// kDebug adds the optional skip_mask_out / margin_out parity outputs.
+template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug>
 __global__ void __launch_bounds__(kNumThreads, 1)
 sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                        const __grid_constant__ CUtensorMap tm_v, const FwdArgs a) {
-    using L = SmemLayout<D, BC, NSTAGE>;
+    using L = SmemLayout<D, BC, NK, NV>;
     static_assert(D == 64 || D == 128, "head dim");
     static_assert(BC == 64 || BC == 128, "key tile");
     static_assert(2 * BC + 2 * D <= kTmemCols, "TMEM budget");
@@ -92,18 +119,23 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     uint8_t* smem = smem_raw + (sbase - raw);
 
     const uint32_t q_smem = sbase + L::kQOff;
-    const uint32_t kv_smem = sbase + L::kKVOff;
+    const uint32_t k_smem = sbase + L::kKOff;
+    const uint32_t v_smem = sbase + L::kVOff;
     const uint32_t bar0 = sbase + L::kBarOff;
     auto q_full = [&](int x) { return bar0 + 8u * x; };
-    auto kv_full = [&](int s) { return bar0 + 8u * (2 + s); };
-    auto kv_empty = [&](int s) { return bar0 + 8u * (2 + NSTAGE + s); };
-    auto s_full = [&](int x) { return bar0 + 8u * (2 + 2 * NSTAGE + x); };
-    auto p_ready = [&](int x) { return bar0 + 8u * (4 + 2 * NSTAGE + x); };
-    auto o_full = [&](int x) { return bar0 + 8u * (6 + 2 * NSTAGE + x); };
+    auto k_full = [&](int s) { return bar0 + 8u * (2 + s); };
+    auto k_empty = [&](int s) { return bar0 + 8u * (2 + NK + s); };
+    auto v_full = [&](int s) { return bar0 + 8u * (2 + 2 * NK + s); };
+    auto v_empty = [&](int s) { return bar0 + 8u * (2 + 2 * NK + NV + s); };
+    constexpr int kB = 2 + 2 * NK + 2 * NV;
+    auto s_full = [&](int x) { return bar0 + 8u * (kB + x); };        // S_X(j) complete in TMEM
+    auto p_half = [&](int x) { return bar0 + 8u * (kB + 2 + x); };    // first half of P_X written (kept tiles only)
+    auto p_ready = [&](int x) { return bar0 + 8u * (kB + 4 + x); };   // all of P_X written (kept tiles only)
+    auto o_full = [&](int x) { return bar0 + 8u * (kB + 6 + x); };    // last P V of slot X complete
+    auto dec = [&](int x) { return bar0 + 8u * (kB + 10 + x); };      // the 4 warps of slot X have voted on tile j
     volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + L::kMiscOff);
-    volatile int* keepflag = reinterpret_cast<volatile int*>(smem + L::kMiscOff + 4);          // [2][2]
-    volatile int* votes = reinterpret_cast<volatile int*>(smem + L::kMiscOff + 4 + 16);        // [2][2][4]
-    volatile float* wmax = reinterpret_cast<volatile float*>(smem + L::kMiscOff + 4 + 16 + 64);  // [2][2][4]
+    volatile int* votes = reinterpret_cast<volatile int*>(smem + L::kMiscOff + 48);              // [2][2][4]
+    volatile float* wmax = reinterpret_cast<volatile float*>(smem + L::kMiscOff + 112);          // [2][2][4]
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -114,20 +146,21 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     const int T_c = a.T_c;
 
     // ------------------------------------------------------------------ setup
-    if (warp == kProducerWarp && lane == 0) {
+    if (warp == kKProducerWarp && lane == 0) {
         prefetch_tmap(&tm_q);
         prefetch_tmap(&tm_k);
         prefetch_tmap(&tm_v);
         for (int x = 0; x < 2; ++x) {
             mbar_init(q_full(x), 1);
             mbar_init(s_full(x), 1);
+            mbar_init(p_half(x), 128);
             mbar_init(p_ready(x), 128);
             mbar_init(o_full(x), 1);
+            mbar_init(dec(x), 4);
         }
-        for (int s = 0; s < NSTAGE; ++s) {
-            mbar_init(kv_full(s), 1);
-            mbar_init(kv_empty(s), 1);
-        }
+        for (int s = 0; s < NK; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
+        for (int s = 0; s < NV; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
+        for (int i = 0; i < 16; ++i) votes[i] = -1;
         fence_mbar_init();
     }
     if (warp == kMmaWarp) {
@@ -141,93 +174,188 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
-        if (warp == kProducerWarp) {
-        // ============================================================== TMA producer (a1)
-        if (lane == 0) {
-            for (int x = 0; x < nX; ++x) {
-                mbar_arrive_expect_tx(q_full(x), L::kQSlotBytes);
-                for (int h = 0; h < kSubD; ++h)
-                    tma_load_3d(q_smem + x * L::kQSlotBytes + h * L::kSubQBytes, &tm_q, h * 64, (tile0 + x) * 128, bh,
-                                q_full(x));
+        // Producer / MMA warps: the whole warp runs each loop (warp-uniform control flow, every lane waits on
+        // the mbarriers) and one elected lane issues, so that descriptors and addresses stay in uniform registers.
+        if (warp == kKProducerWarp) {
+            // ========================================================== Q and K producer (a1)
+            if (elect_one_sync()) {
+                for (int x = 0; x < nX; ++x) {
+                    mbar_arrive_expect_tx(q_full(x), L::kQSlotBytes);
+                    for (int h = 0; h < kSubD; ++h)
+                        tma_load_3d(q_smem + x * L::kQSlotBytes + h * L::kSubQBytes, &tm_q, h * 64,
+                                    (tile0 + x) * 128, bh, q_full(x));
+                }
             }
+            __syncwarp();
             int stage = 0;
             uint32_t phase = 0;
-            for (int e = 0; e < 2 * T_c; ++e) {       // ring entries: K_0, V_0, K_1, V_1, ...
-                if (e >= NSTAGE) mbar_wait(kv_empty(stage), phase ^ 1u);
-                mbar_arrive_expect_tx(kv_full(stage), L::kKVStageBytes);
-                const CUtensorMap* tm = (e & 1) ? &tm_v : &tm_k;
-                for (int h = 0; h < kSubD; ++h)
-                    tma_load_3d(kv_smem + stage * L::kKVStageBytes + h * L::kSubKVBytes, tm, h * 64, (e >> 1) * BC, bh,
-                                kv_full(stage));
-                if (++stage == NSTAGE) { stage = 0; phase ^= 1u; }
+            for (int j = 0; j < T_c; ++j) {
+                if (j >= NK) mbar_wait(k_empty(stage), phase ^ 1u);
+                if (elect_one_sync()) {
+                    mbar_arrive_expect_tx(k_full(stage), L::kKVStageBytes);
+                    for (int h = 0; h < kSubD; ++h)
+                        tma_load_3d(k_smem + stage * L::kKVStageBytes + h * L::kSubKVBytes, &tm_k, h * 64, j * BC, bh,
+                                    k_full(stage));
+                }
+                __syncwarp();
+                if (++stage == NK) { stage = 0; phase ^= 1u; }
             }
-        }
-        __syncwarp();
+        } else if (warp == kVProducerWarp) {
+            // ========================================================== V producer (a1)
+            int slot = 0, nloaded = 0;
+            uint32_t phase = 0;
+            auto load_v = [&](int j) {
+                if (nloaded >= NV) mbar_wait(v_empty(slot), phase ^ 1u);
+                if (elect_one_sync()) {
+                    mbar_arrive_expect_tx(v_full(slot), L::kKVStageBytes);
+                    for (int h = 0; h < kSubD; ++h)
+                        tma_load_3d(v_smem + slot * L::kKVStageBytes + h * L::kSubKVBytes, &tm_v, h * 64, j * BC, bh,
+                                    v_full(slot));
+                }
+                __syncwarp();
+                ++nloaded;
+                if (++slot == NV) { slot = 0; phase ^= 1u; }
+            };
+            // Dense mode only: every V_j is fetched.  In the sparse modes the MMA warp, which is the first to know
+            // a tile's decision, issues the V loads itself (see below) and this warp stays idle.
+            if (!kSparse) {
+                for (int j = 0; j < T_c; ++j) load_v(j);
+            }
         } else if (warp == kMmaWarp) {
-        // ============================================================== MMA issuer (a2, a6)
-        if (lane == 0) {
-            auto issue_qk = [&](int x, uint32_t kaddr) {
+            // ========================================================== MMA issuer (a2, a6)
+            auto issue_qk = [&](int x, uint32_t kaddr, int j = 1000) {
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
                     const uint32_t off = (kk >> 2) * L::kSubQBytes + (kk & 3) * 32;
                     const uint32_t koff = (kk >> 2) * L::kSubKVBytes + (kk & 3) * 32;
                     umma_ss(tmem_base + x * BC, umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
                             umma_smem_desc_sw128(kaddr + koff, 16, 1024), kIdescQK, kk > 0);
+#ifdef DSA_PROF
+                    if (a.prof && blockIdx.x == 0 && blockIdx.y == 0 && j < 32 && (kk == 0 || kk == 1 || kk == 3 || kk == 5 || kk == 7))
+                        a.prof[(1 << 20) + (j * 2 + x) * 16 + 10 + (kk + 1) / 2] = clock64();
+#endif
                 }
             };
-            auto issue_pv = [&](int x, uint32_t vaddr, bool acc) {
+            auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int half) {   // half 0 / 1: keys [0, BC/2) / [BC/2, BC)
 #pragma unroll
-                for (int kk = 0; kk < BC / 16; ++kk) {
+                for (int kk = half * (BC / 32); kk < (half + 1) * (BC / 32); ++kk) {
                     // 16 keys = 16 rows of 128 B; d sub-tiles (64 columns) are L::kSubKVBytes apart (LBO)
                     umma_ts(tmem_base + 2 * BC + x * D, tmem_base + x * BC + kk * 8,
                             umma_smem_desc_sw128(vaddr + kk * 2048, L::kSubKVBytes, 1024), kIdescPV, acc || kk > 0);
                 }
             };
-            int stage = 0;
-            uint32_t phase = 0;
-            auto advance = [&]() { if (++stage == NSTAGE) { stage = 0; phase ^= 1u; } };
+            int kstage = 0, vslot = 0;
+            uint32_t kphase = 0, vphase = 0;
 
+            PROF_DECL(8)
             for (int x = 0; x < nX; ++x) mbar_wait(q_full(x), 0);
-            mbar_wait(kv_full(stage), phase);
+            mbar_wait(k_full(0), 0);
+            PROF_TICK(0)
             tc_fence_after();
-            for (int x = 0; x < nX; ++x) {
-                issue_qk(x, kv_smem + stage * L::kKVStageBytes);
-                umma_commit(s_full(x));
-            }
-            umma_commit(kv_empty(stage));
-            advance();
-
-            for (int j = 0; j < T_c; ++j) {
-                const int v_stage = stage;
-                const uint32_t v_phase = phase;
-                advance();
-                const bool has_next = (j + 1) < T_c;
-                const int k_stage = stage;
-                const uint32_t k_phase = phase;
-                if (has_next) advance();
-                bool v_waited = false, k_waited = false;
+            if (elect_one_sync()) {
                 for (int x = 0; x < nX; ++x) {
-                    mbar_wait(p_ready(x), j & 1);
-                    tc_fence_after();
-                    const int keep = kSparse ? keepflag[x * 2 + (j & 1)] : 1;
-                    if (keep) {
-                        if (!v_waited) { mbar_wait(kv_full(v_stage), v_phase); tc_fence_after(); v_waited = true; }
-                        issue_pv(x, kv_smem + v_stage * L::kKVStageBytes, j > 0);
-                    }
-                    if (has_next) {
-                        if (!k_waited) { mbar_wait(kv_full(k_stage), k_phase); tc_fence_after(); k_waited = true; }
-                        issue_qk(x, kv_smem + k_stage * L::kKVStageBytes);
-                        umma_commit(s_full(x));
-                    } else {
-                        umma_commit(o_full(x));
-                    }
+                    issue_qk(x, k_smem);
+                    umma_commit(s_full(x));
                 }
-                if (!v_waited) mbar_wait(kv_full(v_stage), v_phase);
-                umma_commit(kv_empty(v_stage));
-                if (has_next) umma_commit(kv_empty(k_stage));
+                umma_commit(k_empty(0));
             }
-        }
-        __syncwarp();
+            __syncwarp();
+            if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
+
+            uint32_t ppar[2] = {0u, 0u};                     // parity of p_half / p_ready: they advance on kept tiles only
+            // Sparse modes: this warp also fetches V.  V_j is prefetched when tile j-1 needed its V (decisions are
+            // strongly correlated along j); otherwise it is fetched only once a slot has voted to keep tile j.
+            int lslot = 0, nloaded = 0;                      // V ring, producer side
+            uint32_t lphase = 0;
+            auto load_v = [&](int j) {
+                if (nloaded >= NV) mbar_wait(v_empty(lslot), lphase ^ 1u);
+                if (elect_one_sync()) {
+                    mbar_arrive_expect_tx(v_full(lslot), L::kKVStageBytes);
+                    for (int h = 0; h < kSubD; ++h)
+                        tma_load_3d(v_smem + lslot * L::kKVStageBytes + h * L::kSubKVBytes, &tm_v, h * 64, j * BC, bh,
+                                    v_full(lslot));
+                }
+                __syncwarp();
+                ++nloaded;
+                if (++lslot == NV) { lslot = 0; lphase ^= 1u; }
+            };
+            bool v_loaded = !kSparse;                        // is V_j in (or on its way to) slot vslot?
+            if (kSparse) { load_v(0); v_loaded = true; }     // tile 0 is always kept
+            for (int j = 0; j < T_c; ++j) {
+                const int par = j & 1;
+                const bool has_next = (j + 1) < T_c;
+                bool need = false, v_waited = false;
+                const uint32_t vaddr = v_smem + vslot * L::kKVStageBytes;
+                const uint32_t kaddr = k_smem + kstage * L::kKVStageBytes;
+                PROF_TICK(1)
+                if (has_next) { mbar_wait(k_full(kstage), kphase); tc_fence_after(); }   // K_{j+1} has landed
+                PROF_TICK(5)
+                for (int x = 0; x < nX; ++x) {
+                    bool keep = true;
+                    if (kSparse) {
+                        TRACE(0)
+                        mbar_wait(dec(x), par);              // all 4 warps of slot x have read S_x(j) and voted
+                        tc_fence_after();
+                        TRACE(1)
+                        PROF_TICK(2 + x)
+                        const int tag_keep = (j << 2) | 2;
+                        const int4 vt = lds128_volatile(sbase + L::kMiscOff + 48 + (x * 2 + par) * 16);
+                        keep = (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
+                        need = need || keep;
+                        PROF_TICK(6)
+                        if (keep && !v_loaded) { load_v(j); v_loaded = true; }   // not prefetched: fetch V_j now
+                        PROF_TICK(7)
+                    }
+                    if (keep) {
+                        mbar_wait(p_half(x), ppar[x]);
+                        tc_fence_after();
+                        PROF_TICK(2 + x)
+                        if (!v_waited) { mbar_wait(v_full(vslot), vphase); tc_fence_after(); v_waited = true; }
+                        PROF_TICK(4)
+                        if (elect_one_sync()) issue_pv(x, vaddr, j > 0, 0);
+                        __syncwarp();
+                        PROF_TICK(1)
+                        mbar_wait(p_ready(x), ppar[x]);
+                        tc_fence_after();
+                        ppar[x] ^= 1u;
+                        PROF_TICK(2 + x)
+                    }
+                    TRACE(2)
+                    if (elect_one_sync()) {
+                        if (keep) issue_pv(x, vaddr, true, 1);
+                        if (has_next) {
+                            issue_qk(x, kaddr, j);
+                            umma_commit(s_full(x));
+#ifdef DSA_PROF
+                            if (a.prof && blockIdx.x == 0 && blockIdx.y == 0 && j < 32) a.prof[(1 << 20) + (j * 2 + x) * 16 + 15] = clock64();
+#endif
+                        } else {
+                            umma_commit(o_full(x));
+                        }
+                    }
+                    __syncwarp();
+                    TRACE(3)
+                    PROF_TICK(1)
+                }
+                if (v_loaded) {                              // a V slot was filled for this tile: release it
+                    if (!v_waited) mbar_wait(v_full(vslot), vphase);
+                    if (elect_one_sync()) umma_commit(v_empty(vslot));
+                    __syncwarp();
+                    if (++vslot == NV) { vslot = 0; vphase ^= 1u; }
+                }
+                PROF_TICK(4)
+                if (has_next) {
+                    if (elect_one_sync()) umma_commit(k_empty(kstage));
+                    __syncwarp();
+                    if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
+                }
+                if (kSparse) {
+                    v_loaded = false;
+                    if (need && has_next) { load_v(j + 1); v_loaded = true; }   // prefetch V_{j+1}
+                }
+                PROF_TICK(7)
+            }
+            PROF_FLUSH(0, 8, lane == 0)
         }
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
@@ -255,16 +383,24 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         float m_used = -INFINITY;   // stabiliser actually subtracted (log2 domain, may lag the true max)
         float m_true = -INFINITY;   // running max over retained tiles (log2 domain) -- FIXED mode reference
         float l = 0.f;              // sum over retained tiles of 2^(s - m_used)
+        float lse2 = -INFINITY;     // m_used + log2(l): LSE over retained tiles, log2 domain (Eq. 6) -- DYNAMIC reference
         int n_exec = 0, n_skip = 0;
+        PROF_DECL(8)
 
         for (int j = 0; j < T_c; ++j) {
             const int par = j & 1;
+            PROF_TICK(0)
+            if (w == 0) { TRACE(4) }
             mbar_wait(s_full(x), par);
             tc_fence_after();
+            if (w == 0) { TRACE(5) }
+            PROF_TICK(1)
             uint32_t su[BC / 32][32];                         // this thread's row of S_ij (fp32 bits)
 #pragma unroll
             for (int c = 0; c < BC / 32; ++c) tmem_ld_x32(tS + c * 32, su[c]);
             tmem_wait_ld();
+            if (w == 0) { TRACE(6) }
+            PROF_TICK(2)
 #define S_AT(c) __uint_as_float(su[(c) >> 5][(c) & 31])
             const int valid_cols = a.N - j * BC;             // ragged last K tile: columns beyond N are -inf
             if (valid_cols < BC) {
@@ -272,48 +408,76 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 for (int c = 0; c < BC; ++c)
                     if (c >= valid_cols) su[c >> 5][c & 31] = 0xff800000u;
             }
-            float mx0 = S_AT(0), mx1 = S_AT(1), mx2 = S_AT(2), mx3 = S_AT(3);   // 4 independent max chains
+            float mx0 = S_AT(0), mx1 = S_AT(1), mx2 = S_AT(2), mx3 = S_AT(3);   // 4 independent 3-input max chains
 #pragma unroll
-            for (int c = 4; c < BC; c += 4) {
-                mx0 = fmaxf(mx0, S_AT(c));
-                mx1 = fmaxf(mx1, S_AT(c + 1));
-                mx2 = fmaxf(mx2, S_AT(c + 2));
-                mx3 = fmaxf(mx3, S_AT(c + 3));
+            for (int c = 4; c + 8 <= BC; c += 8) {
+                mx0 = fmax3(mx0, S_AT(c), S_AT(c + 1));
+                mx1 = fmax3(mx1, S_AT(c + 2), S_AT(c + 3));
+                mx2 = fmax3(mx2, S_AT(c + 4), S_AT(c + 5));
+                mx3 = fmax3(mx3, S_AT(c + 6), S_AT(c + 7));
             }
+            mx0 = fmax3(mx0, S_AT(BC - 4), S_AT(BC - 3));
+            mx1 = fmax3(mx1, S_AT(BC - 2), S_AT(BC - 1));
             const float mhat2 = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;   // tile-local row max (a3)
+            if (w == 0) { TRACE(7) }
+            PROF_TICK(3)
 
             // ---- predicate and all-rows vote (a4)
             bool skip_grp = false, keep_any = true;
             float grp_margin = INFINITY;
-            if (kSparse && j > 0) {
-                const float ref = (mode == kModeDynamic) ? (m_used + fast_log2(l)) : m_true;
-                const float t2 = mhat2 - ref;                // Eq. 5 in log2 units
-                const bool row_skip = !row_valid || (t2 < lambda_log2);
-                const int wskip = __all_sync(0xffffffffu, row_skip);
-                if (want_margin) {
-                    float tm = row_valid ? t2 : -INFINITY;
+            if (kSparse) {
+                // votes[x][j & 1][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
+                // The MMA warp combines the four votes itself (barrier dec, one arrival per warp), so an all-skip
+                // decision reaches the tensor pipe without the four warps first synchronising with each other.
+                const float ref = (mode == kModeDynamic) ? lse2 : m_true;
+                const float t2 = mhat2 - ref;                // Eq. 5 in log2 units (+inf at j = 0: tile 0 is kept)
+                const bool row_skip = (j > 0) && (!row_valid || (t2 < lambda_log2));
+                const bool wskip = __all_sync(0xffffffffu, row_skip);
+                volatile int* vt = votes + (x * 2 + par) * 4;   // double-buffered by tile parity
+                tc_fence_before();                           // S_x(j) is in registers: the MMA warp may overwrite it
+                if (lane == 0) {
+                    vt[w] = (j << 2) | (wskip ? 1 : 2);
+                    mbar_arrive(dec(x));
+                }
+                __syncwarp();
+                if (w == 0) { TRACE(8) }
+                if (kDebug) {
+                    if (want_margin) {
+                        float tm = row_valid ? t2 : -INFINITY;
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, o));
-                    if (lane == 0) wmax[(x * 2 + par) * 4 + w] = tm;
-                }
-                if (lane == 0) votes[(x * 2 + par) * 4 + w] = wskip;
-                named_bar_sync(1 + x, 128);
-                const int v0 = votes[(x * 2 + par) * 4 + 0], v1 = votes[(x * 2 + par) * 4 + 1];
-                const int v2 = votes[(x * 2 + par) * 4 + 2], v3 = votes[(x * 2 + par) * 4 + 3];
-                if (G == 1) {
-                    skip_grp = v0 && v1 && v2 && v3;
-                    keep_any = !skip_grp;
-                    if (want_margin)
-                        grp_margin = fmaxf(fmaxf(wmax[(x * 2 + par) * 4 + 0], wmax[(x * 2 + par) * 4 + 1]),
-                                           fmaxf(wmax[(x * 2 + par) * 4 + 2], wmax[(x * 2 + par) * 4 + 3]));
+                        for (int o = 16; o > 0; o >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, o));
+                        if (lane == 0) wmax[(x * 2 + par) * 4 + w] = tm;
+                    }
+                    named_bar_sync(1 + x, 128);
+                    const bool s0 = (vt[0] & 3) == 1, s1 = (vt[1] & 3) == 1, s2 = (vt[2] & 3) == 1, s3 = (vt[3] & 3) == 1;
+                    if (G == 1) {
+                        skip_grp = s0 && s1 && s2 && s3;
+                        keep_any = !skip_grp;
+                        if (want_margin)
+                            grp_margin = fmaxf(fmaxf(wmax[(x * 2 + par) * 4 + 0], wmax[(x * 2 + par) * 4 + 1]),
+                                               fmaxf(wmax[(x * 2 + par) * 4 + 2], wmax[(x * 2 + par) * 4 + 3]));
+                    } else {
+                        skip_grp = grp ? (s2 && s3) : (s0 && s1);
+                        keep_any = !(s0 && s1 && s2 && s3);
+                        if (want_margin)
+                            grp_margin = fmaxf(wmax[(x * 2 + par) * 4 + 2 * grp], wmax[(x * 2 + par) * 4 + 2 * grp + 1]);
+                    }
+                    if (want_margin) grp_margin = (j == 0) ? INFINITY : (grp_margin - lambda_log2) * kLn2;
+                    named_bar_sync(1 + x, 128);              // wmax / votes are reused by the next tile
+                } else if (!wskip) {
+                    skip_grp = false;                        // a row of this warp keeps the tile: no need to wait
+                    keep_any = true;
                 } else {
-                    const bool s0 = v0 && v1, s1 = v2 && v3;
-                    skip_grp = grp ? s1 : s0;
-                    keep_any = !(s0 && s1);
-                    if (want_margin)
-                        grp_margin = fmaxf(wmax[(x * 2 + par) * 4 + 2 * grp], wmax[(x * 2 + par) * 4 + 2 * grp + 1]);
+                    // every row of this warp is below the threshold: wait (hardware-suspended, no shared-memory
+                    // polling) until all four warps have voted on tile j, then read the four votes at once
+                    mbar_wait(dec(x), par);
+                    const int tag_keep = (j << 2) | 2;
+                    const int4 v4 = lds128_volatile(sbase + L::kMiscOff + 48 + (x * 2 + par) * 16);
+                    const bool k0 = v4.x == tag_keep, k1 = v4.y == tag_keep, k2 = v4.z == tag_keep, k3 = v4.w == tag_keep;
+                    keep_any = k0 | k1 | k2 | k3;
+                    if (G == 1) skip_grp = !keep_any;
+                    else skip_grp = !((w >> 1) ? (k2 | k3) : (k0 | k1));
                 }
-                if (want_margin) grp_margin = (grp_margin - lambda_log2) * kLn2;
             }
             if (grp_leader && grp_valid) {                   // a9 + optional parity outputs
                 if (skip_grp) ++n_skip; else ++n_exec;
@@ -322,11 +486,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     if (want_margin) a.margin[tile_row + j] = grp_margin;
                 }
             }
-
+            if (w == 0) { TRACE(9) }
+            PROF_TICK(4)
             if (kSparse && !keep_any) {                      // a7: skipped -- m, l, O untouched
-                if (r == 0) keepflag[x * 2 + par] = 0;
-                tc_fence_before();
-                mbar_arrive(p_ready(x));
+                PROF_TICK(5)
                 continue;
             }
 
@@ -337,6 +500,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 for (int i = 0; i < 16; ++i) z[i] = 0u;
 #pragma unroll
                 for (int c = 0; c < BC / 32; ++c) tmem_st_x16(tS + c * 16, z);
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(p_half(x));
             } else {
                 // ---- online softmax update (a5)
                 if (j == 0) {
@@ -366,22 +532,34 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     uint32_t pk[16];
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
-                        const float p0 = fast_exp2(fmaf(__uint_as_float(su[c][2 * i]), scale_log2, neg_m));
-                        const float p1 = fast_exp2(fmaf(__uint_as_float(su[c][2 * i + 1]), scale_log2, neg_m));
+                        const float x0 = fmaf(__uint_as_float(su[c][2 * i]), scale_log2, neg_m);
+                        const float x1 = fmaf(__uint_as_float(su[c][2 * i + 1]), scale_log2, neg_m);
+                        const bool emul = kEmulPairs >= 8 ? ((i & 1) == 1 && (i >> 1) < kEmulPairs)
+                                                          : ((i & 3) == 3 && (i >> 2) < kEmulPairs);
+                        const float p0 = emul ? exp2_fma(x0) : fast_exp2(x0);
+                        const float p1 = emul ? exp2_fma(x1) : fast_exp2(x1);
                         rs0 += p0;
                         rs1 += p1;
                         pk[i] = pack_bf16x2(p0, p1);
                     }
                     tmem_st_x16(tS + c * 16, pk);
+                    if (c == BC / 64 - 1) {                  // first half of P_X is in TMEM: its P V MMAs may start
+                        tmem_wait_st();
+                        tc_fence_before();
+                        mbar_arrive(p_half(x));
+                    }
                 }
                 l += rs0 + rs1;
+                if (kSparse) lse2 = m_used + fast_log2(l);
             }
 #undef S_AT
+            PROF_TICK(6)
             tmem_wait_st();
             tc_fence_before();
-            if (kSparse && r == 0) keepflag[x * 2 + par] = 1;
             mbar_arrive(p_ready(x));
+            PROF_TICK(7)
         }
+        PROF_FLUSH(8 + 8 * x, 8, r == 0)
 
         // ---- epilogue (a8): O / l -> bf16, lse = ln(l) + m over retained tiles
         mbar_wait(o_full(x), 0);

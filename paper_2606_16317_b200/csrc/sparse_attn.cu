@@ -11,6 +11,14 @@
 
 #include "fwd_kernel.cuh"
 
+// K / V ring depths of the D = 128 kernels (Q 64 KB + (NK + NV) x 32 KB must fit in 227 KB)
+#ifndef DSA_NK
+#define DSA_NK 3
+#endif
+#ifndef DSA_NV
+#define DSA_NV 2
+#endif
+
 namespace {
 
 thread_local char g_last_error[512] = "";
@@ -63,11 +71,11 @@ int make_tmap(EncodeTiledFn enc, CUtensorMap* tm, const void* base, int BH, int 
     return 0;
 }
 
-template <int D, int BC, int G, int NSTAGE, bool kSparse, bool kDebug>
+template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug>
 int launch(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const dsa::FwdArgs& args, int BH,
            cudaStream_t stream) {
-    using L = dsa::SmemLayout<D, BC, NSTAGE>;
-    auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NSTAGE, kSparse, kDebug>;
+    using L = dsa::SmemLayout<D, BC, NK, NV>;
+    auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NK, NV, kSparse, kDebug>;
     static bool configured = false;
     if (!configured) {
         CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L::kDynamicBytes));
@@ -176,20 +184,23 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     a.mode = mode;
     a.scale_log2 = r.scale * dsa::kLog2e;
     a.lambda_log2 = r.lambda * dsa::kLog2e;
+#ifdef DSA_PROF
+    a.prof = reinterpret_cast<unsigned long long*>(getenv("DSA_PROF_PTR") ? strtoull(getenv("DSA_PROF_PTR"), nullptr, 0) : 0ull);
+#endif
 
     if (stats_out) CUDA_TRY(cudaMemsetAsync(stats_out, 0, sizeof(int64_t) * 2 * BH, r.stream));
     const bool sparse = mode != SPARSE_ATTN_DENSE;
     const bool debug = r.skip_mask || r.margin;
     if (D == 128) {
-        if (!sparse && !debug) return launch<128, 128, 1, 4, false, false>(tq, tk, tv, a, BH, r.stream);
-        if (!sparse) return launch<128, 128, 1, 4, false, true>(tq, tk, tv, a, BH, r.stream);
-        if (!debug) return launch<128, 128, 1, 4, true, false>(tq, tk, tv, a, BH, r.stream);
-        return launch<128, 128, 1, 4, true, true>(tq, tk, tv, a, BH, r.stream);
+        if (!sparse && !debug) return launch<128, 128, 1, DSA_NK, DSA_NV, false, false>(tq, tk, tv, a, BH, r.stream);
+        if (!sparse) return launch<128, 128, 1, DSA_NK, DSA_NV, false, true>(tq, tk, tv, a, BH, r.stream);
+        if (!debug) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false>(tq, tk, tv, a, BH, r.stream);
+        return launch<128, 128, 1, DSA_NK, DSA_NV, true, true>(tq, tk, tv, a, BH, r.stream);
     }
-    if (!sparse && !debug) return launch<64, 64, 2, 4, false, false>(tq, tk, tv, a, BH, r.stream);
-    if (!sparse) return launch<64, 64, 2, 4, false, true>(tq, tk, tv, a, BH, r.stream);
-    if (!debug) return launch<64, 64, 2, 4, true, false>(tq, tk, tv, a, BH, r.stream);
-    return launch<64, 64, 2, 4, true, true>(tq, tk, tv, a, BH, r.stream);
+    if (!sparse && !debug) return launch<64, 64, 2, 3, 2, false, false>(tq, tk, tv, a, BH, r.stream);
+    if (!sparse) return launch<64, 64, 2, 3, 2, false, true>(tq, tk, tv, a, BH, r.stream);
+    if (!debug) return launch<64, 64, 2, 3, 2, true, false>(tq, tk, tv, a, BH, r.stream);
+    return launch<64, 64, 2, 3, 2, true, true>(tq, tk, tv, a, BH, r.stream);
 }
 
 int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse, int B, int H, int N, int D,
