@@ -249,9 +249,9 @@ def main():
                 t = torch.tensor([total], device="cuda")
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
                 total = float(t.item())
-                gathered = [torch.zeros_like(stats) for _ in range(world)]
-                dist.all_gather(gathered, torch.from_numpy(st).cuda())     # [world][B,H,2]: per-head counts
-                st_all = torch.stack(gathered).cpu().numpy()
+                from paper_2606_16317_b200.sharding import gather_stats
+                # every rank owns cfg.H heads of the (world * H)-head job: assemble the per-head counts
+                st_all = gather_stats(torch.from_numpy(st).cuda(), cfg.H * world).cpu().numpy()[None]
             else:
                 st_all = st[None]
             ms = total / args.steps
