@@ -32,6 +32,9 @@ from workloads import CONFIGS, make_qkv  # noqa: E402
 METRIC = "attention ms & effective TFLOP/s vs dense mode at Wan-2.2 shapes; sparsity %; % tensor peak"
 P_REAL = 1.5            # Eq. 7 "transition region" constant
 FALLBACK_TFLOPS = 1590.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one DENSE config-1 launch, ncu --set full (profiles/ncu_dense_r01.md);
+# algorithmic bytes: q + k + v + out + lse = 4 * 201.3 MB + 3.1 MB = 808 MB
+NCU_DRAM_BYTES_DENSE_CFG1 = 608.49e6 + 187.54e6
 
 
 def measured_peaks():
@@ -336,7 +339,7 @@ def main():
                                      "of": f"{tb} TFLOP/s ({peak_kind} burst)"},
         "modes": results,
         "roofline": {"bound": "tensor", "achieved": ach, "peak": tb, "unit": "TFLOP/s", "frac": ach / tb,
-                     "traffic": None, "kernel": "sparse_attn_fwd_kernel<128,128,1,*> DENSE mode",
+                     "traffic": NCU_DRAM_BYTES_DENSE_CFG1 if args.config == "cfg1" else None, "kernel": "sparse_attn_fwd_kernel<128,128,1,*> DENSE mode",
                      "peak_kind": f"{peak_kind} bf16 burst; sustained {ts}", "frac_sustained": ach / ts,
                      "frac_dynamic_mode": ach_dyn / tb,
                      "flop_per_launch": dense_res["executed_flop_per_launch_rank0"],
