@@ -43,10 +43,13 @@ constexpr int kNumThreads = 384;      // 3 warpgroups
 constexpr int kKProducerWarp = 8;
 constexpr int kMmaWarp = 9;
 constexpr int kVProducerWarp = 10;
-// setmaxnreg: the kernel launches with 168 registers/thread (65536 / 384); the two softmax warpgroups
-// grow to 224 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 56.
-constexpr int kRegsSoftmax = 224;
-constexpr int kRegsOther = 56;
+// setmaxnreg: the kernel launches with 168 registers/thread (65536 / 384); the two softmax warpgroups grow to
+// 208 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 88.  The registers the 128
+// threads give up must cover what the 256 softmax threads take, or setmaxnreg.inc never returns.
+constexpr int kRegsLaunch = 168;
+constexpr int kRegsSoftmax = 208;
+constexpr int kRegsOther = 88;
+static_assert((kRegsLaunch - kRegsOther) * 128 >= (kRegsSoftmax - kRegsLaunch) * 256, "setmaxnreg pool imbalance");
 constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -88,10 +91,10 @@ struct SmemLayout {
     static constexpr int kVOff = kKOff + NK * kKVStageBytes;
     static constexpr int kBarOff = kVOff + NV * kKVStageBytes;
     // barriers (8 B each): q_full[2] k_full[NK] k_empty[NK] v_full[NV] v_empty[NV]
-    //                      s_full[2] p_half[2] p_ready[2] o_full[2] (2 unused) dec[2]
-    static constexpr int kNumBars = 2 + 2 * NK + 2 * NV + 8 + 2 + 2;
+    //                      s_full[2] p_half[2] p_ready[2] o_full[2] s_read[2] dec[2][2] vcmd[NV]
+    static constexpr int kNumBars = 2 + 2 * NK + 2 * NV + 8 + 2 + 4 + NV;
     static constexpr int kMiscOff = kBarOff + 8 * kNumBars;
-    // misc: tmem_ptr (4) | pad (44) | votes[2][2][4] (64) | wmax[2][2][4] (64)
+    // misc: tmem_ptr (4) | pad (12) | vcmd[NV] (<= 32) | votes[2][2][4] (64) | wmax[2][2][4] (64)
     static constexpr int kMiscBytes = 16 + 16 + 16 + 64 + 64;
     static constexpr int kTotal = kMiscOff + kMiscBytes;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
@@ -132,7 +135,13 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     auto p_half = [&](int x) { return bar0 + 8u * (kB + 2 + x); };    // first half of P_X written (kept tiles only)
     auto p_ready = [&](int x) { return bar0 + 8u * (kB + 4 + x); };   // all of P_X written (kept tiles only)
     auto o_full = [&](int x) { return bar0 + 8u * (kB + 6 + x); };    // last P V of slot X complete
-    auto dec = [&](int x) { return bar0 + 8u * (kB + 10 + x); };      // the 4 warps of slot X have voted on tile j
+    auto s_read = [&](int x) { return bar0 + 8u * (kB + 8 + x); };    // the 4 warps of slot X hold S_X(j) in registers
+    // the 4 warps of slot X have voted on tile j.  One barrier per tile parity: inside a run of skipped tiles the
+    // softmax warps may vote on tile j+1 (its S was issued speculatively) before the MMA warp has looked at the
+    // votes of tile j, and a single barrier two phases ahead of its waiter would alias.
+    auto dec = [&](int x, int par) { return bar0 + 8u * (kB + 10 + 2 * x + par); };
+    auto vcmd_bar = [&](int s) { return bar0 + 8u * (kB + 14 + s); }; // sparse modes: "load V_j into slot s" posted
+    volatile int* vcmd = reinterpret_cast<volatile int*>(smem + L::kMiscOff + 16);               // [NV]
     volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + L::kMiscOff);
     volatile int* votes = reinterpret_cast<volatile int*>(smem + L::kMiscOff + 48);              // [2][2][4]
     volatile float* wmax = reinterpret_cast<volatile float*>(smem + L::kMiscOff + 112);          // [2][2][4]
@@ -156,8 +165,11 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             mbar_init(p_half(x), 128);
             mbar_init(p_ready(x), 128);
             mbar_init(o_full(x), 1);
-            mbar_init(dec(x), 4);
+            mbar_init(dec(x, 0), 4);
+            mbar_init(dec(x, 1), 4);
+            mbar_init(s_read(x), 4);
         }
+        for (int s = 0; s < NV; ++s) mbar_init(vcmd_bar(s), 1);
         for (int s = 0; s < NK; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
         for (int s = 0; s < NV; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
         for (int i = 0; i < 16; ++i) votes[i] = -1;
@@ -216,16 +228,33 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 ++nloaded;
                 if (++slot == NV) { slot = 0; phase ^= 1u; }
             };
-            // Dense mode only: every V_j is fetched.  In the sparse modes the MMA warp, which is the first to know
-            // a tile's decision, issues the V loads itself (see below) and this warp stays idle.
+            // Dense mode: every V_j is fetched.  Sparse modes: the MMA warp, which is the first to know a tile's
+            // decision, posts "load V_j" commands (one mbarrier + one word per ring slot) and this warp executes
+            // them, so that waiting for a free slot never stalls the tensor-pipe issuer.  j < 0 ends the loop.
             if (!kSparse) {
                 for (int j = 0; j < T_c; ++j) load_v(j);
+            } else {
+                int cslot = 0;
+                uint32_t cphase = 0;
+                while (true) {
+                    mbar_wait(vcmd_bar(cslot), cphase);
+                    const int j = vcmd[cslot];
+                    if (j < 0) break;
+                    load_v(j);
+                    if (++cslot == NV) { cslot = 0; cphase ^= 1u; }
+                }
             }
         } else if (warp == kMmaWarp) {
             // ========================================================== MMA issuer (a2, a6)
             auto issue_qk = [&](int x, uint32_t kaddr, int j = 1000) {
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
+#if defined(DSA_EXP) && (DSA_EXP & 8)
+                    if (kk >= 4) break;
+#endif
+#if defined(DSA_EXP) && (DSA_EXP & 16)
+                    if (kk >= 1) break;
+#endif
                     const uint32_t off = (kk >> 2) * L::kSubQBytes + (kk & 3) * 32;
                     const uint32_t koff = (kk >> 2) * L::kSubKVBytes + (kk & 3) * 32;
                     umma_ss(tmem_base + x * BC, umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
@@ -263,47 +292,69 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
 
             uint32_t ppar[2] = {0u, 0u};                     // parity of p_half / p_ready: they advance on kept tiles only
-            // Sparse modes: this warp also fetches V.  V_j is prefetched when tile j-1 needed its V (decisions are
-            // strongly correlated along j); otherwise it is fetched only once a slot has voted to keep tile j.
-            int lslot = 0, nloaded = 0;                      // V ring, producer side
-            uint32_t lphase = 0;
-            auto load_v = [&](int j) {
-                if (nloaded >= NV) mbar_wait(v_empty(lslot), lphase ^ 1u);
+            // Sparse modes.  (1) V: tile j's V is requested (from the V warp) once some slot has voted to keep tile j,
+            // and V_{j+1} right after it (decisions are strongly correlated along j).  (2) Speculation: inside a run
+            // of skipped tiles the next S_x(j+1) = Q_x K_{j+1}^T is issued as soon as the softmax warps hold S_x(j) in
+            // registers (barrier s_read), without waiting for their vote: the vote is then off the critical chain.
+            // If tile j turns out to be kept, the softmax warps let the speculative MMA finish before they write P_x
+            // over it, and S_x(j+1) is issued again after P_x V_j.  Scheduling only: no decision depends on it.
+            int lslot = 0;                                   // V ring, command side
+            auto post_v = [&](int j) {
                 if (elect_one_sync()) {
-                    mbar_arrive_expect_tx(v_full(lslot), L::kKVStageBytes);
-                    for (int h = 0; h < kSubD; ++h)
-                        tma_load_3d(v_smem + lslot * L::kKVStageBytes + h * L::kSubKVBytes, &tm_v, h * 64, j * BC, bh,
-                                    v_full(lslot));
+                    vcmd[lslot] = j;
+                    mbar_arrive(vcmd_bar(lslot));
                 }
                 __syncwarp();
-                ++nloaded;
-                if (++lslot == NV) { lslot = 0; lphase ^= 1u; }
+                if (++lslot == NV) lslot = 0;
             };
             bool v_loaded = !kSparse;                        // is V_j in (or on its way to) slot vslot?
-            if (kSparse) { load_v(0); v_loaded = true; }     // tile 0 is always kept
+            bool v_next = false;                             // has V_{j+1} been requested?
+            bool prev_skip[2] = {false, false};              // did slot x skip tile j-1?
+            if (kSparse) { post_v(0); v_loaded = true; }     // tile 0 is always kept
             for (int j = 0; j < T_c; ++j) {
                 const int par = j & 1;
                 const bool has_next = (j + 1) < T_c;
-                bool need = false, v_waited = false;
+                bool v_waited = false;
                 const uint32_t vaddr = v_smem + vslot * L::kKVStageBytes;
                 const uint32_t kaddr = k_smem + kstage * L::kKVStageBytes;
                 PROF_TICK(1)
                 if (has_next) { mbar_wait(k_full(kstage), kphase); tc_fence_after(); }   // K_{j+1} has landed
                 PROF_TICK(5)
+                bool spec[2] = {false, false};
+                if (kSparse) {
+                    for (int x = 0; x < nX; ++x) {
+                        spec[x] = prev_skip[x] && has_next;
+                        if (spec[x]) {
+                            mbar_wait(s_read(x), par);       // S_x(j) is in the softmax warps' registers
+                            tc_fence_after();
+                            if (elect_one_sync()) {
+                                issue_qk(x, kaddr, j);
+                                umma_commit(s_full(x));
+                            }
+                            __syncwarp();
+                        }
+                    }
+                    PROF_TICK(6)
+                }
                 for (int x = 0; x < nX; ++x) {
                     bool keep = true;
+#if defined(DSA_EXP) && (DSA_EXP & 2)
+                    if (kSparse && spec[x]) { keep = false; } else
+#endif
                     if (kSparse) {
                         TRACE(0)
-                        mbar_wait(dec(x), par);              // all 4 warps of slot x have read S_x(j) and voted
+                        mbar_wait(dec(x, par), (j >> 1) & 1);              // all 4 warps of slot x have voted on tile j
                         tc_fence_after();
                         TRACE(1)
                         PROF_TICK(2 + x)
                         const int tag_keep = (j << 2) | 2;
                         const int4 vt = lds128_volatile(sbase + L::kMiscOff + 48 + (x * 2 + par) * 16);
                         keep = (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
-                        need = need || keep;
-                        PROF_TICK(6)
-                        if (keep && !v_loaded) { load_v(j); v_loaded = true; }   // not prefetched: fetch V_j now
+                        prev_skip[x] = !keep;
+                        if (keep) {
+                            if (!v_loaded) { post_v(j); v_loaded = true; }                 // not prefetched: fetch V_j now
+                            if (!v_next && has_next) { post_v(j + 1); v_next = true; }     // and prefetch V_{j+1}
+                        }
                         PROF_TICK(7)
                     }
                     if (keep) {
@@ -321,19 +372,18 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         PROF_TICK(2 + x)
                     }
                     TRACE(2)
-                    if (elect_one_sync()) {
-                        if (keep) issue_pv(x, vaddr, true, 1);
-                        if (has_next) {
-                            issue_qk(x, kaddr, j);
-                            umma_commit(s_full(x));
-#ifdef DSA_PROF
-                            if (a.prof && blockIdx.x == 0 && blockIdx.y == 0 && j < 32) a.prof[(1 << 20) + (j * 2 + x) * 16 + 15] = clock64();
-#endif
-                        } else {
-                            umma_commit(o_full(x));
+                    if (keep || !spec[x]) {
+                        if (elect_one_sync()) {
+                            if (keep) issue_pv(x, vaddr, true, 1);
+                            if (has_next) {
+                                issue_qk(x, kaddr, j);       // (again, if the speculative one was overwritten by P_x)
+                                umma_commit(s_full(x));
+                            } else {
+                                umma_commit(o_full(x));
+                            }
                         }
+                        __syncwarp();
                     }
-                    __syncwarp();
                     TRACE(3)
                     PROF_TICK(1)
                 }
@@ -349,12 +399,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     __syncwarp();
                     if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
                 }
-                if (kSparse) {
-                    v_loaded = false;
-                    if (need && has_next) { load_v(j + 1); v_loaded = true; }   // prefetch V_{j+1}
-                }
-                PROF_TICK(7)
+                if (kSparse) { v_loaded = v_next; v_next = false; }
             }
+            if (kSparse) post_v(-1);                         // every requested V has been consumed: stop the V warp
             PROF_FLUSH(0, 8, lane == 0)
         }
     } else {
@@ -385,13 +432,17 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         float l = 0.f;              // sum over retained tiles of 2^(s - m_used)
         float lse2 = -INFINITY;     // m_used + log2(l): LSE over retained tiles, log2 domain (Eq. 6) -- DYNAMIC reference
         int n_exec = 0, n_skip = 0;
+        uint32_t sfpar = 0;         // parity of s_full(x): one phase per S_x issued (two for a tile re-issued after a
+                                    // mis-speculated skip)
+        bool prev_skip = false;     // did this slot skip tile j-1?
         PROF_DECL(8)
 
         for (int j = 0; j < T_c; ++j) {
             const int par = j & 1;
             PROF_TICK(0)
             if (w == 0) { TRACE(4) }
-            mbar_wait(s_full(x), par);
+            mbar_wait(s_full(x), sfpar);
+            sfpar ^= 1u;
             tc_fence_after();
             if (w == 0) { TRACE(5) }
             PROF_TICK(1)
@@ -399,6 +450,12 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 #pragma unroll
             for (int c = 0; c < BC / 32; ++c) tmem_ld_x32(tS + c * 32, su[c]);
             tmem_wait_ld();
+            // inside a run of skipped tiles the MMA warp issues S_x(j+1) as soon as S_x(j) has left TMEM
+            const bool spec = kSparse && prev_skip && (j + 1) < T_c;
+            if (kSparse) {
+                tc_fence_before();
+                if (lane == 0) mbar_arrive(s_read(x));
+            }
             if (w == 0) { TRACE(6) }
             PROF_TICK(2)
 #define S_AT(c) __uint_as_float(su[(c) >> 5][(c) & 31])
@@ -418,7 +475,11 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
             mx0 = fmax3(mx0, S_AT(BC - 4), S_AT(BC - 3));
             mx1 = fmax3(mx1, S_AT(BC - 2), S_AT(BC - 1));
+#if defined(DSA_EXP) && (DSA_EXP & 1)
+            const float mhat2 = S_AT(0) * scale_log2;
+#else
             const float mhat2 = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;   // tile-local row max (a3)
+#endif
             if (w == 0) { TRACE(7) }
             PROF_TICK(3)
 
@@ -437,7 +498,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 tc_fence_before();                           // S_x(j) is in registers: the MMA warp may overwrite it
                 if (lane == 0) {
                     vt[w] = (j << 2) | (wskip ? 1 : 2);
-                    mbar_arrive(dec(x));
+                    mbar_arrive(dec(x, par));
                 }
                 __syncwarp();
                 if (w == 0) { TRACE(8) }
@@ -470,7 +531,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 } else {
                     // every row of this warp is below the threshold: wait (hardware-suspended, no shared-memory
                     // polling) until all four warps have voted on tile j, then read the four votes at once
-                    mbar_wait(dec(x), par);
+#if defined(DSA_EXP) && (DSA_EXP & 4)
+                    if (j < 2)
+#endif
+                    mbar_wait(dec(x, par), (j >> 1) & 1);
                     const int tag_keep = (j << 2) | 2;
                     const int4 v4 = lds128_volatile(sbase + L::kMiscOff + 48 + (x * 2 + par) * 16);
                     const bool k0 = v4.x == tag_keep, k1 = v4.y == tag_keep, k2 = v4.z == tag_keep, k3 = v4.w == tag_keep;
@@ -488,9 +552,17 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
             if (w == 0) { TRACE(9) }
             PROF_TICK(4)
+            prev_skip = kSparse && !keep_any;
             if (kSparse && !keep_any) {                      // a7: skipped -- m, l, O untouched
                 PROF_TICK(5)
                 continue;
+            }
+            if (spec) {
+                // tile j is kept although a speculative S_x(j+1) is being written over S_x: let that MMA finish before
+                // P_x goes into the same columns (the MMA warp issues S_x(j+1) again after P_x V_j)
+                mbar_wait(s_full(x), sfpar);
+                sfpar ^= 1u;
+                tc_fence_after();
             }
 
             if (kSparse && G == 2 && skip_grp) {
