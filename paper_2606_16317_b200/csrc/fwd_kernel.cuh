@@ -26,10 +26,22 @@
 namespace dsa {
 
 #ifdef DSA_PROF
+#if DSA_PROF == 2   // timeline of CTA (0, 0) only, no per-phase accumulators
+#define PROF_DECL(n)
+#define PROF_TICK(i)
+#define PROF_FLUSH(base, n, cond)
+#else
 #define PROF_DECL(n) unsigned long long prof_acc[n] = {}; long long prof_t = clock64();
 #define PROF_TICK(i) { long long t__ = clock64(); prof_acc[i] += t__ - prof_t; prof_t = t__; }
 #define PROF_FLUSH(base, n, cond) if (a.prof && (cond)) { for (int i__ = 0; i__ < n; ++i__) a.prof[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * 32 + base + i__] = prof_acc[i__]; }
-#define TRACE(slot) if (a.prof && blockIdx.x == 0 && blockIdx.y == 0 && j < 32 && (threadIdx.x & 31) == 0) a.prof[(1 << 20) + (j * 2 + x) * 16 + (slot)] = clock64();
+#endif
+#define TRACE(slot) if (a.prof && blockIdx.x == DSA_TRACE_CTA && blockIdx.y == 0 && j >= DSA_TRACE_J0 && j < DSA_TRACE_J0 + 32 && (threadIdx.x & 31) == 0) a.prof[(1 << 20) + ((j - DSA_TRACE_J0) * 2 + x) * 16 + (slot)] = clock64();
+#ifndef DSA_TRACE_CTA
+#define DSA_TRACE_CTA 0
+#endif
+#ifndef DSA_TRACE_J0
+#define DSA_TRACE_J0 0
+#endif
 #else
 #define TRACE(slot)
 #define PROF_DECL(n)
@@ -260,8 +272,8 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     umma_ss(tmem_base + x * BC, umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
                             umma_smem_desc_sw128(kaddr + koff, 16, 1024), kIdescQK, kk > 0);
 #ifdef DSA_PROF
-                    if (a.prof && blockIdx.x == 0 && blockIdx.y == 0 && j < 32 && (kk == 0 || kk == 1 || kk == 3 || kk == 5 || kk == 7))
-                        a.prof[(1 << 20) + (j * 2 + x) * 16 + 10 + (kk + 1) / 2] = clock64();
+                    if (a.prof && blockIdx.x == DSA_TRACE_CTA && blockIdx.y == 0 && j >= DSA_TRACE_J0 && j < DSA_TRACE_J0 + 32 && (kk == 0 || kk == 7))
+                        a.prof[(1 << 20) + ((j - DSA_TRACE_J0) * 2 + x) * 16 + 10 + (kk + 1) / 2] = clock64();
 #endif
                 }
             };
@@ -319,6 +331,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const uint32_t kaddr = k_smem + kstage * L::kKVStageBytes;
                 PROF_TICK(1)
                 if (has_next) { mbar_wait(k_full(kstage), kphase); tc_fence_after(); }   // K_{j+1} has landed
+                { const int x = 0; TRACE(11) }
                 PROF_TICK(5)
                 bool spec[2] = {false, false};
                 if (kSparse) {
@@ -326,12 +339,14 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         spec[x] = prev_skip[x] && has_next;
                         if (spec[x]) {
                             mbar_wait(s_read(x), par);       // S_x(j) is in the softmax warps' registers
+                            TRACE(12)
                             tc_fence_after();
                             if (elect_one_sync()) {
                                 issue_qk(x, kaddr, j);
                                 umma_commit(s_full(x));
                             }
                             __syncwarp();
+                            TRACE(13)
                         }
                     }
                     PROF_TICK(6)
