@@ -7,10 +7,14 @@
 //   warps 0-3   softmax warpgroup of slot 0 (thread <-> query row <-> TMEM lane)
 //   warps 4-7   softmax warpgroup of slot 1
 //   warp  8     TMA producer for Q (once) and the K ring (runs ahead of the decisions)
-//   warp  9     tcgen05.mma issuer (one elected lane) and TMEM owner
-//   warp  10    TMA producer for the V ring in DENSE mode (in the sparse modes the MMA warp fetches V_j itself,
-//               and only if some slot keeps tile j or tile j-1 needed its V)
-//   warp  11    idle (completes the third warpgroup so that setmaxnreg can hand its registers over)
+//   warp  9     tcgen05.mma issuer of slot 0 (one elected lane) and TMEM owner
+//   warp  10    TMA producer for the V ring: slot j % NV holds V_j.  DENSE: every tile.  Sparse modes: this warp
+//               reads both slots' votes on tile j and fetches V_j only if some slot keeps tile j (plus V_{j+1}
+//               speculatively after a kept tile); an unneeded tile completes its ring phase without a load
+//   warp  11    tcgen05.mma issuer of slot 1
+// One issuer warp per slot: a thread that issues tcgen05.mma is held until its last MMA has been dispatched to the
+// tensor pipe, so with a single issuer every barrier wait and vote decode of one slot left the pipe idle; with two,
+// the control work of one slot overlaps the MMAs of the other.
 // TMEM (512 columns): S_0 | S_1 (fp32, BC columns each; P_X, bf16x2, aliases the first BC/2 columns of S_X)
 //                     O_0 | O_1 (fp32, D columns each).
 // Per slot X and K tile j:  S_X = Q_X K_j^T (always)  ->  softmax warpgroup: row max, skip predicate,
@@ -35,7 +39,7 @@ namespace dsa {
 #define PROF_TICK(i) { long long t__ = clock64(); prof_acc[i] += t__ - prof_t; prof_t = t__; }
 #define PROF_FLUSH(base, n, cond) if (a.prof && (cond)) { for (int i__ = 0; i__ < n; ++i__) a.prof[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * 32 + base + i__] = prof_acc[i__]; }
 #endif
-#define TRACE(slot) if (a.prof && blockIdx.x == DSA_TRACE_CTA && blockIdx.y == 0 && j >= DSA_TRACE_J0 && j < DSA_TRACE_J0 + 32 && (threadIdx.x & 31) == 0) a.prof[(1 << 20) + ((j - DSA_TRACE_J0) * 2 + x) * 16 + (slot)] = clock64();
+#define TRACE(slot) if (a.prof && blockIdx.x == DSA_TRACE_CTA && blockIdx.y == 0 && j >= DSA_TRACE_J0 && j < DSA_TRACE_J0 + 32 && (threadIdx.x & 31) == 0) a.prof[(1 << 20) + ((j - DSA_TRACE_J0) * 2 + x) * 32 + (slot)] = clock64();
 #ifndef DSA_TRACE_CTA
 #define DSA_TRACE_CTA 0
 #endif
@@ -53,8 +57,9 @@ enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2 };
 
 constexpr int kNumThreads = 384;      // 3 warpgroups
 constexpr int kKProducerWarp = 8;
-constexpr int kMmaWarp = 9;
+constexpr int kMmaWarp0 = 9;
 constexpr int kVProducerWarp = 10;
+constexpr int kMmaWarp1 = 11;
 // setmaxnreg: the kernel launches with 168 registers/thread (65536 / 384); the two softmax warpgroups grow to
 // 208 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 88.  The registers the 128
 // threads give up must cover what the 256 softmax threads take, or setmaxnreg.inc never returns.
@@ -73,6 +78,22 @@ constexpr float kRescaleThreshold = 8.0f;
 #define DSA_EMUL_PAIRS 0
 #endif
 constexpr int kEmulPairs = DSA_EMUL_PAIRS;
+#ifndef DSA_EXP
+#define DSA_EXP 0   // timing experiments only (results are wrong unless nothing is skipped)
+#endif
+#ifndef DSA_EXP_LOCK
+#define DSA_EXP_LOCK 0
+#endif
+// number of tcgen05.mma issuer warps (1: warp 9 drives both slots; 2: one warp per slot)
+#ifndef DSA_GATE
+#define DSA_GATE 1
+#endif
+#ifndef DSA_ISSUERS_DENSE
+#define DSA_ISSUERS_DENSE 1
+#endif
+#ifndef DSA_ISSUERS_SPARSE
+#define DSA_ISSUERS_SPARSE 2
+#endif
 
 struct FwdArgs {
     __nv_bfloat16* out;          // [BH, N, D]
@@ -103,11 +124,14 @@ struct SmemLayout {
     static constexpr int kVOff = kKOff + NK * kKVStageBytes;
     static constexpr int kBarOff = kVOff + NV * kKVStageBytes;
     // barriers (8 B each): q_full[2] k_full[NK] k_empty[NK] v_full[NV] v_empty[NV]
-    //                      s_full[2] p_half[2] p_ready[2] o_full[2] s_read[2] dec[2][2] vcmd[NV]
-    static constexpr int kNumBars = 2 + 2 * NK + 2 * NV + 8 + 2 + 4 + NV;
+    //                      s_full[2] p_half[2] p_ready[2] o_full[2] s_read[2] dec[2][4]
+    static constexpr int kNumBars = 2 + 2 * NK + 2 * NV + 8 + 2 + 8;
     static constexpr int kMiscOff = kBarOff + 8 * kNumBars;
-    // misc: tmem_ptr (4) | pad (12) | vcmd[NV] (<= 32) | votes[2][2][4] (64) | wmax[2][2][4] (64)
-    static constexpr int kMiscBytes = 16 + 16 + 16 + 64 + 64;
+    // misc: tmem_ptr (4) | pad (12) | votes[2][4][4] (128) | wmax[2][4][4] (128) | in_exp[2][4] (32) | prog[2] (16)
+    static constexpr int kVotesOff = kMiscOff + 16;
+    static constexpr int kLockOff = kVotesOff + 256;
+    static constexpr int kProgOff = kLockOff + 32;
+    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16;
     static constexpr int kTotal = kMiscOff + kMiscBytes;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
     static_assert(kDynamicBytes <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
@@ -148,15 +172,14 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     auto p_ready = [&](int x) { return bar0 + 8u * (kB + 4 + x); };   // all of P_X written (kept tiles only)
     auto o_full = [&](int x) { return bar0 + 8u * (kB + 6 + x); };    // last P V of slot X complete
     auto s_read = [&](int x) { return bar0 + 8u * (kB + 8 + x); };    // the 4 warps of slot X hold S_X(j) in registers
-    // the 4 warps of slot X have voted on tile j.  One barrier per tile parity: inside a run of skipped tiles the
-    // softmax warps may vote on tile j+1 (its S was issued speculatively) before the MMA warp has looked at the
-    // votes of tile j, and a single barrier two phases ahead of its waiter would alias.
-    auto dec = [&](int x, int par) { return bar0 + 8u * (kB + 10 + 2 * x + par); };
-    auto vcmd_bar = [&](int s) { return bar0 + 8u * (kB + 14 + s); }; // sparse modes: "load V_j into slot s" posted
-    volatile int* vcmd = reinterpret_cast<volatile int*>(smem + L::kMiscOff + 16);               // [NV]
+    // the 4 warps of slot X have voted on tile j.  A ring of 4 barriers (and 4 vote words per warp), indexed by
+    // j & 3: the votes are read by the slot's MMA warp, by the V warp and by the slot's own all-skip warps.  Slot x
+    // can only vote on tile j + 3 after its MMA warp has finished tile j + 1, which waits for v_full of tile j + 1,
+    // which the V warp completes only after it has read every vote on tile j: a ring of 4 can never be lapped.
+    auto dec = [&](int x, int q) { return bar0 + 8u * (kB + 10 + 4 * x + q); };
     volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + L::kMiscOff);
-    volatile int* votes = reinterpret_cast<volatile int*>(smem + L::kMiscOff + 48);              // [2][2][4]
-    volatile float* wmax = reinterpret_cast<volatile float*>(smem + L::kMiscOff + 112);          // [2][2][4]
+    volatile int* votes = reinterpret_cast<volatile int*>(smem + L::kVotesOff);                  // [2][4][4]
+    volatile float* wmax = reinterpret_cast<volatile float*>(smem + L::kVotesOff + 128);         // [2][4][4]
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -177,17 +200,18 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             mbar_init(p_half(x), 128);
             mbar_init(p_ready(x), 128);
             mbar_init(o_full(x), 1);
-            mbar_init(dec(x, 0), 4);
-            mbar_init(dec(x, 1), 4);
+            for (int q = 0; q < 4; ++q) mbar_init(dec(x, q), 4);
             mbar_init(s_read(x), 4);
         }
-        for (int s = 0; s < NV; ++s) mbar_init(vcmd_bar(s), 1);
-        for (int s = 0; s < NK; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), 1); }
-        for (int s = 0; s < NV; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), 1); }
-        for (int i = 0; i < 16; ++i) votes[i] = -1;
+        // a K stage is released by one softmax lane per active slot (when S_x of that tile is complete),
+        // a V slot by the MMA warp of every active slot (after its P V, or at once if it skipped the tile)
+        for (int s = 0; s < NK; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), nX); }
+        for (int s = 0; s < NV; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), nX); }
+        for (int i = 0; i < 32; ++i) votes[i] = -1;
+        for (int i = 0; i < 12; ++i) reinterpret_cast<volatile int*>(smem + L::kLockOff)[i] = 0;  // in_exp, prog
         fence_mbar_init();
     }
-    if (warp == kMmaWarp) {
+    if (warp == kMmaWarp0) {
         tmem_alloc(smem_u32(const_cast<uint32_t*>(tmem_ptr)), kTmemCols);
         tmem_relinquish();
     }
@@ -226,10 +250,14 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
         } else if (warp == kVProducerWarp) {
             // ========================================================== V producer (a1)
-            int slot = 0, nloaded = 0;
-            uint32_t phase = 0;
+            // V_j lives in ring slot j % NV, and v_full / v_empty of that slot complete exactly one phase per tile
+            // mapped to it, whether V_j was fetched or not, so every waiter's phase parity is a function of j alone.
+            auto wait_slot_free = [&](int j) {               // tile j - NV has been released by every active slot
+                if (j >= NV) mbar_wait(v_empty(j % NV), static_cast<uint32_t>((j / NV) - 1) & 1u);
+            };
             auto load_v = [&](int j) {
-                if (nloaded >= NV) mbar_wait(v_empty(slot), phase ^ 1u);
+                const int slot = j % NV;
+                wait_slot_free(j);
                 if (elect_one_sync()) {
                     mbar_arrive_expect_tx(v_full(slot), L::kKVStageBytes);
                     for (int h = 0; h < kSubD; ++h)
@@ -237,44 +265,55 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                                     v_full(slot));
                 }
                 __syncwarp();
-                ++nloaded;
-                if (++slot == NV) { slot = 0; phase ^= 1u; }
             };
-            // Dense mode: every V_j is fetched.  Sparse modes: the MMA warp, which is the first to know a tile's
-            // decision, posts "load V_j" commands (one mbarrier + one word per ring slot) and this warp executes
-            // them, so that waiting for a free slot never stalls the tensor-pipe issuer.  j < 0 ends the loop.
-            if (!kSparse) {
+            if (!kSparse || (DSA_EXP & 4)) {
                 for (int j = 0; j < T_c; ++j) load_v(j);
             } else {
-                int cslot = 0;
-                uint32_t cphase = 0;
-                while (true) {
-                    mbar_wait(vcmd_bar(cslot), cphase);
-                    const int j = vcmd[cslot];
-                    if (j < 0) break;
-                    load_v(j);
-                    if (++cslot == NV) { cslot = 0; cphase ^= 1u; }
+                // Sparse modes: V_j is needed iff some slot keeps tile j.  This warp reads the votes of both slots
+                // (barrier dec), fetches V_j if it is needed and not yet there, and after a kept tile fetches V_{j+1}
+                // ahead of its votes (decisions are strongly correlated along j); a wasted prefetch costs L2 traffic
+                // only.  A tile nobody keeps completes its v_full phase with a plain arrive.
+                load_v(0);                                   // tile 0 is always kept
+                bool have = true;                            // is V_j already in (or on its way to) its slot?
+                for (int j = 0; j < T_c; ++j) {
+                    const int q = j & 3;
+                    const int tag_keep = (j << 2) | 2;
+                    const bool has_next = (j + 1) < T_c;
+                    bool have_next = false;
+                    bool keep = false;
+                    for (int x = 0; x < nX; ++x) {           // act on the first keep vote, do not wait for both slots
+                        mbar_wait(dec(x, q), (j >> 2) & 1);
+                        const int4 vt = lds128_volatile(sbase + L::kVotesOff + (x * 4 + q) * 16);
+                        keep |= (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
+                        if (keep) {
+                            if (!have) { load_v(j); have = true; }
+                            if (has_next && !have_next) { load_v(j + 1); have_next = true; }
+                        }
+                    }
+                    if (!have) {                             // nobody keeps tile j: complete its phase without a load
+                        wait_slot_free(j);
+                        if (lane == 0) mbar_arrive(v_full(j % NV));
+                        __syncwarp();
+                    }
+                    have = have_next;
                 }
             }
-        } else if (warp == kMmaWarp) {
-            // ========================================================== MMA issuer (a2, a6)
-            auto issue_qk = [&](int x, uint32_t kaddr, int j = 1000) {
+        } else if (warp == kMmaWarp0 || warp == kMmaWarp1) {
+            // ========================================================== MMA issuer(s) (a2, a6)
+            // kIssuers == 2: warp 9 drives slot 0 and warp 11 slot 1.  kIssuers == 1: warp 9 drives both slots in turn
+            // (warp 11 idles), which forces the two slots into anti-phase -- the best schedule when every tile is kept.
+            constexpr int kIssuers = kSparse ? DSA_ISSUERS_SPARSE : DSA_ISSUERS_DENSE;
+            constexpr bool kGate = kIssuers == 2 && DSA_GATE;
+            const int x_lo = (kIssuers == 2 && warp == kMmaWarp1) ? 1 : 0;
+            const int x_hi = (kIssuers == 2) ? x_lo + 1 : nX;        // this warp drives slots [x_lo, x_hi)
+            if ((kIssuers == 2 || warp == kMmaWarp0) && x_lo < nX) {
+            auto issue_qk = [&](int x, uint32_t kaddr) {
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
-#if defined(DSA_EXP) && (DSA_EXP & 8)
-                    if (kk >= 4) break;
-#endif
-#if defined(DSA_EXP) && (DSA_EXP & 16)
-                    if (kk >= 1) break;
-#endif
                     const uint32_t off = (kk >> 2) * L::kSubQBytes + (kk & 3) * 32;
                     const uint32_t koff = (kk >> 2) * L::kSubKVBytes + (kk & 3) * 32;
                     umma_ss(tmem_base + x * BC, umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
                             umma_smem_desc_sw128(kaddr + koff, 16, 1024), kIdescQK, kk > 0);
-#ifdef DSA_PROF
-                    if (a.prof && blockIdx.x == DSA_TRACE_CTA && blockIdx.y == 0 && j >= DSA_TRACE_J0 && j < DSA_TRACE_J0 + 32 && (kk == 0 || kk == 7))
-                        a.prof[(1 << 20) + ((j - DSA_TRACE_J0) * 2 + x) * 16 + 10 + (kk + 1) / 2] = clock64();
-#endif
                 }
             };
             auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int half) {   // half 0 / 1: keys [0, BC/2) / [BC/2, BC)
@@ -285,139 +324,120 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             umma_smem_desc_sw128(vaddr + kk * 2048, L::kSubKVBytes, 1024), kIdescPV, acc || kk > 0);
                 }
             };
-            int kstage = 0, vslot = 0;
-            uint32_t kphase = 0, vphase = 0;
-
-            PROF_DECL(8)
-            for (int x = 0; x < nX; ++x) mbar_wait(q_full(x), 0);
+            int kstage = 0;
+            uint32_t kphase = 0;
+            for (int x = x_lo; x < x_hi; ++x) mbar_wait(q_full(x), 0);
             mbar_wait(k_full(0), 0);
-            PROF_TICK(0)
             tc_fence_after();
             if (elect_one_sync()) {
-                for (int x = 0; x < nX; ++x) {
+                for (int x = x_lo; x < x_hi; ++x) {
                     issue_qk(x, k_smem);
                     umma_commit(s_full(x));
                 }
-                umma_commit(k_empty(0));
             }
             __syncwarp();
             if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
-
-            uint32_t ppar[2] = {0u, 0u};                     // parity of p_half / p_ready: they advance on kept tiles only
-            // Sparse modes.  (1) V: tile j's V is requested (from the V warp) once some slot has voted to keep tile j,
-            // and V_{j+1} right after it (decisions are strongly correlated along j).  (2) Speculation: inside a run
-            // of skipped tiles the next S_x(j+1) = Q_x K_{j+1}^T is issued as soon as the softmax warps hold S_x(j) in
-            // registers (barrier s_read), without waiting for their vote: the vote is then off the critical chain.
-            // If tile j turns out to be kept, the softmax warps let the speculative MMA finish before they write P_x
-            // over it, and S_x(j+1) is issued again after P_x V_j.  Scheduling only: no decision depends on it.
-            int lslot = 0;                                   // V ring, command side
-            auto post_v = [&](int j) {
-                if (elect_one_sync()) {
-                    vcmd[lslot] = j;
-                    mbar_arrive(vcmd_bar(lslot));
-                }
-                __syncwarp();
-                if (++lslot == NV) lslot = 0;
-            };
-            bool v_loaded = !kSparse;                        // is V_j in (or on its way to) slot vslot?
-            bool v_next = false;                             // has V_{j+1} been requested?
-            bool prev_skip[2] = {false, false};              // did slot x skip tile j-1?
-            if (kSparse) { post_v(0); v_loaded = true; }     // tile 0 is always kept
+            uint32_t ppar[2] = {0u, 0u};                 // parity of p_half / p_ready: they advance on kept tiles only
+            bool prev_skip[2] = {false, false};          // did slot x skip tile j-1?
+            // Sparse modes, speculation: inside a run of skipped tiles the next S_x(j+1) = Q_x K_{j+1}^T is issued as
+            // soon as the softmax warps hold S_x(j) in registers (barrier s_read), without waiting for their vote:
+            // the vote is then off the critical chain.  If tile j turns out to be kept, the softmax warps let the
+            // speculative MMA finish before they write P_x over it, and S_x(j+1) is issued again after P_x V_j.
+            // Scheduling only: no decision depends on it.
             for (int j = 0; j < T_c; ++j) {
-                const int par = j & 1;
                 const bool has_next = (j + 1) < T_c;
-                bool v_waited = false;
+                const int vslot = j % NV;
+                const uint32_t vph = static_cast<uint32_t>(j / NV) & 1u;
                 const uint32_t vaddr = v_smem + vslot * L::kKVStageBytes;
                 const uint32_t kaddr = k_smem + kstage * L::kKVStageBytes;
-                PROF_TICK(1)
                 if (has_next) { mbar_wait(k_full(kstage), kphase); tc_fence_after(); }   // K_{j+1} has landed
-                { const int x = 0; TRACE(11) }
-                PROF_TICK(5)
                 bool spec[2] = {false, false};
                 if (kSparse) {
-                    for (int x = 0; x < nX; ++x) {
+#pragma unroll
+                    for (int x = 0; x < 2; ++x) {
+                        if (x < x_lo || x >= x_hi) continue;
                         spec[x] = prev_skip[x] && has_next;
                         if (spec[x]) {
-                            mbar_wait(s_read(x), par);       // S_x(j) is in the softmax warps' registers
+                            mbar_wait(s_read(x), j & 1);     // S_x(j) is in the softmax warps' registers
                             TRACE(12)
                             tc_fence_after();
                             if (elect_one_sync()) {
-                                issue_qk(x, kaddr, j);
+                                issue_qk(x, kaddr);
                                 umma_commit(s_full(x));
                             }
                             __syncwarp();
                             TRACE(13)
                         }
                     }
-                    PROF_TICK(6)
                 }
-                for (int x = 0; x < nX; ++x) {
+#pragma unroll
+                for (int x = 0; x < 2; ++x) {
+                    if (x < x_lo || x >= x_hi) continue;
                     bool keep = true;
-#if defined(DSA_EXP) && (DSA_EXP & 2)
-                    if (kSparse && spec[x]) { keep = false; } else
-#endif
-                    if (kSparse) {
+                    if (kSparse && !(DSA_EXP & 2)) {
                         TRACE(0)
-                        mbar_wait(dec(x, par), (j >> 1) & 1);              // all 4 warps of slot x have voted on tile j
-                        tc_fence_after();
+                        const int q = j & 3;
+                        mbar_wait(dec(x, q), (j >> 2) & 1);  // all 4 warps of slot x have voted on tile j
+                        tc_fence_after();                    // (their votes follow their tcgen05.ld of S_x(j))
                         TRACE(1)
-                        PROF_TICK(2 + x)
                         const int tag_keep = (j << 2) | 2;
-                        const int4 vt = lds128_volatile(sbase + L::kMiscOff + 48 + (x * 2 + par) * 16);
+                        const int4 vt = lds128_volatile(sbase + L::kVotesOff + (x * 4 + q) * 16);
                         keep = (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
                         prev_skip[x] = !keep;
-                        if (keep) {
-                            if (!v_loaded) { post_v(j); v_loaded = true; }                 // not prefetched: fetch V_j now
-                            if (!v_next && has_next) { post_v(j + 1); v_next = true; }     // and prefetch V_{j+1}
-                        }
-                        PROF_TICK(7)
+                    }
+                    if (kGate && nX == 2 && keep) {
+                        // two issuers: the P V phases of two slots that both keep their tiles still take turns in the
+                        // order (0, j), (1, j), (0, j+1), ... as they would with one issuer, which holds the slots in
+                        // anti-phase (softmax of one under the MMAs of the other); a slot that skips never waits, and
+                        // the speculative issues above run side by side.  Scheduling only.
+                        const int need = (x == 0) ? j : j + 1;
+                        while (static_cast<int>(ld_shared_u32(sbase + L::kProgOff + 4 * (1 - x))) < need) { }
                     }
                     if (keep) {
                         mbar_wait(p_half(x), ppar[x]);
-                        tc_fence_after();
-                        PROF_TICK(2 + x)
-                        if (!v_waited) { mbar_wait(v_full(vslot), vphase); tc_fence_after(); v_waited = true; }
-                        PROF_TICK(4)
+                        mbar_wait(v_full(vslot), vph);       // V_j has landed (sparse modes: fetched by the V warp
+                        tc_fence_after();                    // once some slot voted to keep tile j, or prefetched)
                         if (elect_one_sync()) issue_pv(x, vaddr, j > 0, 0);
                         __syncwarp();
-                        PROF_TICK(1)
                         mbar_wait(p_ready(x), ppar[x]);
                         tc_fence_after();
                         ppar[x] ^= 1u;
-                        PROF_TICK(2 + x)
-                    }
-                    TRACE(2)
-                    if (keep || !spec[x]) {
+                        TRACE(2)
                         if (elect_one_sync()) {
-                            if (keep) issue_pv(x, vaddr, true, 1);
+                            issue_pv(x, vaddr, true, 1);
+                            umma_commit(v_empty(vslot));     // this slot's P_x V_j has read V_j
                             if (has_next) {
-                                issue_qk(x, kaddr, j);       // (again, if the speculative one was overwritten by P_x)
+                                issue_qk(x, kaddr);          // (again, if the speculative one was overwritten by P_x)
                                 umma_commit(s_full(x));
                             } else {
                                 umma_commit(o_full(x));
                             }
                         }
                         __syncwarp();
+                    } else {
+                        TRACE(2)
+                        if (!spec[x]) {
+                            if (elect_one_sync()) {
+                                if (has_next) {
+                                    issue_qk(x, kaddr);
+                                    umma_commit(s_full(x));
+                                } else {
+                                    umma_commit(o_full(x));
+                                }
+                            }
+                            __syncwarp();
+                        }
+                        // the V warp has dealt with tile j (and a prefetched but unused V_j has landed): release the slot
+                        mbar_wait(v_full(vslot), vph);
+                        if (lane == 0) mbar_arrive(v_empty(vslot));
+                        __syncwarp();
                     }
+                    if (kGate && nX == 2 && lane == 0) st_shared_u32(sbase + L::kProgOff + 4 * x, static_cast<uint32_t>(j + 1));
                     TRACE(3)
-                    PROF_TICK(1)
                 }
-                if (v_loaded) {                              // a V slot was filled for this tile: release it
-                    if (!v_waited) mbar_wait(v_full(vslot), vphase);
-                    if (elect_one_sync()) umma_commit(v_empty(vslot));
-                    __syncwarp();
-                    if (++vslot == NV) { vslot = 0; vphase ^= 1u; }
-                }
-                PROF_TICK(4)
-                if (has_next) {
-                    if (elect_one_sync()) umma_commit(k_empty(kstage));
-                    __syncwarp();
-                    if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
-                }
-                if (kSparse) { v_loaded = v_next; v_next = false; }
+                if (has_next && ++kstage == NK) { kstage = 0; kphase ^= 1u; }
             }
-            if (kSparse) post_v(-1);                         // every requested V has been consumed: stop the V warp
-            PROF_FLUSH(0, 8, lane == 0)
+            }
         }
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsSoftmax));
@@ -442,6 +462,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         const float lambda_log2 = a.lambda_log2;
         const bool want_margin = kDebug && a.margin != nullptr;
 
+        constexpr bool kUseExpLock = DSA_EXP_LOCK == 2 || (DSA_EXP_LOCK == 1 && (kSparse ? DSA_ISSUERS_SPARSE : DSA_ISSUERS_DENSE) == 2);
         float m_used = -INFINITY;   // stabiliser actually subtracted (log2 domain, may lag the true max)
         float m_true = -INFINITY;   // running max over retained tiles (log2 domain) -- FIXED mode reference
         float l = 0.f;              // sum over retained tiles of 2^(s - m_used)
@@ -453,12 +474,14 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         PROF_DECL(8)
 
         for (int j = 0; j < T_c; ++j) {
-            const int par = j & 1;
             PROF_TICK(0)
             if (w == 0) { TRACE(4) }
             mbar_wait(s_full(x), sfpar);
             sfpar ^= 1u;
             tc_fence_after();
+            // S_x(j) is complete, so this slot's Q K^T has read K_j for the last time (a mis-speculated S_x(j) was
+            // consumed, and issued again, during tile j-1): release this slot's hold on the K stage
+            if (w == 0 && lane == 0) mbar_arrive(k_empty(j % NK));
             if (w == 0) { TRACE(5) }
             PROF_TICK(1)
             uint32_t su[BC / 32][32];                         // this thread's row of S_ij (fp32 bits)
@@ -467,7 +490,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             tmem_wait_ld();
             // inside a run of skipped tiles the MMA warp issues S_x(j+1) as soon as S_x(j) has left TMEM
             const bool spec = kSparse && prev_skip && (j + 1) < T_c;
-            if (kSparse) {
+            if (kSparse && !(DSA_EXP & 1)) {
                 tc_fence_before();
                 if (lane == 0) mbar_arrive(s_read(x));
             }
@@ -490,11 +513,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
             mx0 = fmax3(mx0, S_AT(BC - 4), S_AT(BC - 3));
             mx1 = fmax3(mx1, S_AT(BC - 2), S_AT(BC - 1));
-#if defined(DSA_EXP) && (DSA_EXP & 1)
-            const float mhat2 = S_AT(0) * scale_log2;
-#else
             const float mhat2 = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;   // tile-local row max (a3)
-#endif
             if (w == 0) { TRACE(7) }
             PROF_TICK(3)
 
@@ -509,11 +528,12 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const float t2 = mhat2 - ref;                // Eq. 5 in log2 units (+inf at j = 0: tile 0 is kept)
                 const bool row_skip = (j > 0) && (!row_valid || (t2 < lambda_log2));
                 const bool wskip = __all_sync(0xffffffffu, row_skip);
-                volatile int* vt = votes + (x * 2 + par) * 4;   // double-buffered by tile parity
+                const int q = j & 3;
+                volatile int* vt = votes + (x * 4 + q) * 4;     // ring of 4 tiles (see dec)
                 tc_fence_before();                           // S_x(j) is in registers: the MMA warp may overwrite it
-                if (lane == 0) {
+                if (lane == 0 && !(DSA_EXP & 8)) {
                     vt[w] = (j << 2) | (wskip ? 1 : 2);
-                    mbar_arrive(dec(x, par));
+                    mbar_arrive(dec(x, q));
                 }
                 __syncwarp();
                 if (w == 0) { TRACE(8) }
@@ -522,7 +542,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         float tm = row_valid ? t2 : -INFINITY;
 #pragma unroll
                         for (int o = 16; o > 0; o >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, o));
-                        if (lane == 0) wmax[(x * 2 + par) * 4 + w] = tm;
+                        if (lane == 0) wmax[(x * 4 + q) * 4 + w] = tm;
                     }
                     named_bar_sync(1 + x, 128);
                     const bool s0 = (vt[0] & 3) == 1, s1 = (vt[1] & 3) == 1, s2 = (vt[2] & 3) == 1, s3 = (vt[3] & 3) == 1;
@@ -530,13 +550,13 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         skip_grp = s0 && s1 && s2 && s3;
                         keep_any = !skip_grp;
                         if (want_margin)
-                            grp_margin = fmaxf(fmaxf(wmax[(x * 2 + par) * 4 + 0], wmax[(x * 2 + par) * 4 + 1]),
-                                               fmaxf(wmax[(x * 2 + par) * 4 + 2], wmax[(x * 2 + par) * 4 + 3]));
+                            grp_margin = fmaxf(fmaxf(wmax[(x * 4 + q) * 4 + 0], wmax[(x * 4 + q) * 4 + 1]),
+                                               fmaxf(wmax[(x * 4 + q) * 4 + 2], wmax[(x * 4 + q) * 4 + 3]));
                     } else {
                         skip_grp = grp ? (s2 && s3) : (s0 && s1);
                         keep_any = !(s0 && s1 && s2 && s3);
                         if (want_margin)
-                            grp_margin = fmaxf(wmax[(x * 2 + par) * 4 + 2 * grp], wmax[(x * 2 + par) * 4 + 2 * grp + 1]);
+                            grp_margin = fmaxf(wmax[(x * 4 + q) * 4 + 2 * grp], wmax[(x * 4 + q) * 4 + 2 * grp + 1]);
                     }
                     if (want_margin) grp_margin = (j == 0) ? INFINITY : (grp_margin - lambda_log2) * kLn2;
                     named_bar_sync(1 + x, 128);              // wmax / votes are reused by the next tile
@@ -546,12 +566,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 } else {
                     // every row of this warp is below the threshold: wait (hardware-suspended, no shared-memory
                     // polling) until all four warps have voted on tile j, then read the four votes at once
-#if defined(DSA_EXP) && (DSA_EXP & 4)
-                    if (j < 2)
-#endif
-                    mbar_wait(dec(x, par), (j >> 1) & 1);
+                    mbar_wait(dec(x, q), (j >> 2) & 1);
                     const int tag_keep = (j << 2) | 2;
-                    const int4 v4 = lds128_volatile(sbase + L::kMiscOff + 48 + (x * 2 + par) * 16);
+                    const int4 v4 = lds128_volatile(sbase + L::kVotesOff + (x * 4 + q) * 16);
                     const bool k0 = v4.x == tag_keep, k1 = v4.y == tag_keep, k2 = v4.z == tag_keep, k3 = v4.w == tag_keep;
                     keep_any = k0 | k1 | k2 | k3;
                     if (G == 1) skip_grp = !keep_any;
@@ -580,6 +597,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 tc_fence_after();
             }
 
+            float rs0 = 0.f, rs1 = 0.f;                      // this tile's row sum, two chains
             if (kSparse && G == 2 && skip_grp) {
                 // this half skipped but its partner half kept: contribute P = 0, statistics untouched
                 uint32_t z[16];
@@ -612,8 +630,18 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     }
                 }
                 m_true = fmaxf(m_true, mhat2);
+                // Warps w of the two slots share one scheduler, hence one MUFU pipe.  Two exp phases run side by side
+                // both finish late; one after the other, the first finishes early and the second no later.  More
+                // important, with one MMA issuer per slot a free-running pair of slots settles in phase (both in
+                // softmax, then both in MMA), which idles the tensor pipe half of the time.  A warp therefore starts its
+                // exp phase only when its partner is not inside one (a flag per warp, checked then set: no atomics, a
+                // rare double entry is harmless).  That shifts the slots into anti-phase.  Scheduling only.
+                if (kUseExpLock && nX == 2) {
+                    while (ld_shared_u32(sbase + L::kLockOff + 4 * ((1 - x) * 4 + w)) != 0u) { }
+                    st_shared_u32(sbase + L::kLockOff + 4 * (x * 4 + w), 1u);
+                }
+                TRACE(16 + w)
                 const float neg_m = -m_used;
-                float rs0 = 0.f, rs1 = 0.f;
 #pragma unroll
                 for (int c = 0; c < BC / 32; ++c) {          // 32 columns -> 16 packed bf16x2 -> P columns [16c, 16c+16)
                     uint32_t pk[16];
@@ -634,16 +662,23 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         tmem_wait_st();
                         tc_fence_before();
                         mbar_arrive(p_half(x));
+                        TRACE(20 + w)
                     }
                 }
-                l += rs0 + rs1;
-                if (kSparse) lse2 = m_used + fast_log2(l);
+                if (kUseExpLock && nX == 2) st_shared_u32(sbase + L::kLockOff + 4 * (x * 4 + w), 0u);
             }
 #undef S_AT
             PROF_TICK(6)
             tmem_wait_st();
             tc_fence_before();
             mbar_arrive(p_ready(x));
+            TRACE(24 + w)
+            // the statistics are updated after P has been handed over: the tail of the row-sum chain and the log2
+            // must not sit between the last exp and the arrive (in-order issue would stall the arrive on them)
+            if (!(kSparse && G == 2 && skip_grp)) {
+                l += rs0 + rs1;
+                if (kSparse && mode == kModeDynamic && !(DSA_EXP & 16)) lse2 = m_used + fast_log2(l);
+            }
             PROF_TICK(7)
         }
         PROF_FLUSH(8 + 8 * x, 8, r == 0)
@@ -682,7 +717,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     // ------------------------------------------------------------------ teardown
     tc_fence_before();
     __syncthreads();
-    if (warp == kMmaWarp) tmem_dealloc(tmem_base, kTmemCols);
+    if (warp == kMmaWarp0) tmem_dealloc(tmem_base, kTmemCols);
 }
 
 }  // namespace dsa

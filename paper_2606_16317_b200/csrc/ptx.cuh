@@ -60,6 +60,20 @@ __device__ __forceinline__ int4 lds128_volatile(uint32_t saddr) {
     return v;
 }
 
+__device__ __forceinline__ uint32_t atomic_cas_shared(uint32_t saddr, uint32_t cmp, uint32_t val) {
+    uint32_t old;
+    asm volatile("atom.shared.cas.b32 %0, [%1], %2, %3;" : "=r"(old) : "r"(saddr), "r"(cmp), "r"(val) : "memory");
+    return old;
+}
+__device__ __forceinline__ uint32_t ld_shared_u32(uint32_t saddr) {
+    uint32_t v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_shared_u32(uint32_t saddr, uint32_t val) {
+    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(saddr), "r"(val) : "memory");
+}
+
 // ------------------------------------------------------------------ named barriers
 __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
