@@ -72,12 +72,15 @@ constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 // lazy rescale: O and l are only rescaled when the row max grew by more than 2^8 (log2 domain).
 constexpr float kRescaleThreshold = 8.0f;
-// of every 16 (p0, p1) pairs of a 32-column chunk, this many are exponentiated on the FMA pipe (exp2_fma).
-// Measured on B200: the softmax warps are issue-bound, not MUFU-bound, so 0 is fastest.
-#ifndef DSA_EMUL_PAIRS
-#define DSA_EMUL_PAIRS 0
+// Early issue of the second half of S_x(j+1) (keys [BC/2, BC), columns P_x(j) does not use) as soon as S_x(j) is in
+// registers.  Measured slower on B200 (dense cfg1 11.3 ms against 10.1 ms): with A = Q_x read from shared memory every
+// N = BC/2 instruction still reads the whole 4 KB A tile, so two half-width Q K^T cost ~1.5x one full-width one.  Off.
+#ifndef DSA_EARLY_B
+#define DSA_EARLY_B 0
 #endif
-constexpr int kEmulPairs = DSA_EMUL_PAIRS;
+#ifndef DSA_F32X2
+#define DSA_F32X2 1
+#endif
 #ifndef DSA_EXP
 #define DSA_EXP 0   // timing experiments only (results are wrong unless nothing is skipped)
 #endif
@@ -150,6 +153,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     constexpr int BR = 128 / G;
     constexpr int kSubD = D / 64;
     constexpr uint32_t kIdescQK = umma_idesc_bf16(128, BC, 0);   // S = Q K^T: A, B both K-major
+    constexpr uint32_t kIdescQKh = umma_idesc_bf16(128, BC / 2, 0);   // one half of the keys of a tile
     constexpr uint32_t kIdescPV = umma_idesc_bf16(128, D, 1);    // O += P V: B = V is MN-major (d contiguous)
 
     extern __shared__ uint8_t smem_raw[];
@@ -304,16 +308,20 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             // (warp 11 idles), which forces the two slots into anti-phase -- the best schedule when every tile is kept.
             constexpr int kIssuers = kSparse ? DSA_ISSUERS_SPARSE : DSA_ISSUERS_DENSE;
             constexpr bool kGate = kIssuers == 2 && DSA_GATE;
+            constexpr bool kEarlyB = DSA_EARLY_B;
             const int x_lo = (kIssuers == 2 && warp == kMmaWarp1) ? 1 : 0;
             const int x_hi = (kIssuers == 2) ? x_lo + 1 : nX;        // this warp drives slots [x_lo, x_hi)
             if ((kIssuers == 2 || warp == kMmaWarp0) && x_lo < nX) {
-            auto issue_qk = [&](int x, uint32_t kaddr) {
+            // S_x = Q_x K^T for the keys of half h of the tile (h = 0: keys [0, BC/2) -> columns [0, BC/2) of S_x,
+            // h = 1: the other half; h = 2: the whole tile in one N = BC instruction per k step)
+            auto issue_qk = [&](int x, uint32_t kaddr, int h = 2) {
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
                     const uint32_t off = (kk >> 2) * L::kSubQBytes + (kk & 3) * 32;
-                    const uint32_t koff = (kk >> 2) * L::kSubKVBytes + (kk & 3) * 32;
-                    umma_ss(tmem_base + x * BC, umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
-                            umma_smem_desc_sw128(kaddr + koff, 16, 1024), kIdescQK, kk > 0);
+                    const uint32_t koff = (kk >> 2) * L::kSubKVBytes + (kk & 3) * 32 + (h == 1 ? (BC / 2) * 128 : 0);
+                    umma_ss(tmem_base + x * BC + (h == 1 ? BC / 2 : 0),
+                            umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
+                            umma_smem_desc_sw128(kaddr + koff, 16, 1024), h == 2 ? kIdescQK : kIdescQKh, kk > 0);
                 }
             };
             auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int half) {   // half 0 / 1: keys [0, BC/2) / [BC/2, BC)
@@ -351,28 +359,28 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const uint32_t vaddr = v_smem + vslot * L::kKVStageBytes;
                 const uint32_t kaddr = k_smem + kstage * L::kKVStageBytes;
                 if (has_next) { mbar_wait(k_full(kstage), kphase); tc_fence_after(); }   // K_{j+1} has landed
-                bool spec[2] = {false, false};
-                if (kSparse) {
-#pragma unroll
-                    for (int x = 0; x < 2; ++x) {
-                        if (x < x_lo || x >= x_hi) continue;
-                        spec[x] = prev_skip[x] && has_next;
-                        if (spec[x]) {
-                            mbar_wait(s_read(x), j & 1);     // S_x(j) is in the softmax warps' registers
-                            TRACE(12)
-                            tc_fence_after();
-                            if (elect_one_sync()) {
-                                issue_qk(x, kaddr);
-                                umma_commit(s_full(x));
-                            }
-                            __syncwarp();
-                            TRACE(13)
-                        }
-                    }
-                }
 #pragma unroll
                 for (int x = 0; x < 2; ++x) {
                     if (x < x_lo || x >= x_hi) continue;
+                    // As soon as the softmax warps hold S_x(j) in registers (barrier s_read), the second half of
+                    // S_x(j+1) is issued: its columns are not needed for P_x(j), which occupies the first BC/2 columns
+                    // only, so this half of the next Q K^T is off the chain P ready -> P V -> Q K^T -> S ready.
+                    // In a run of skipped tiles the first half follows at once (speculation, see above).
+                    const bool spec = kSparse && prev_skip[x] && has_next;
+                    if (has_next && (kEarlyB || spec)) {
+                        mbar_wait(s_read(x), j & 1);
+                        TRACE(12)
+                        tc_fence_after();
+                        if (elect_one_sync()) {
+                            if (kEarlyB) issue_qk(x, kaddr, 1);
+                            if (spec) {
+                                issue_qk(x, kaddr, kEarlyB ? 0 : 2);
+                                umma_commit(s_full(x));
+                            }
+                        }
+                        __syncwarp();
+                        TRACE(13)
+                    }
                     bool keep = true;
                     if (kSparse && !(DSA_EXP & 2)) {
                         TRACE(0)
@@ -407,7 +415,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             issue_pv(x, vaddr, true, 1);
                             umma_commit(v_empty(vslot));     // this slot's P_x V_j has read V_j
                             if (has_next) {
-                                issue_qk(x, kaddr);          // (again, if the speculative one was overwritten by P_x)
+                                issue_qk(x, kaddr, kEarlyB ? 0 : 2);   // (again, if a speculative one was overwritten by P_x)
                                 umma_commit(s_full(x));
                             } else {
                                 umma_commit(o_full(x));
@@ -416,10 +424,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         __syncwarp();
                     } else {
                         TRACE(2)
-                        if (!spec[x]) {
+                        if (!spec) {
                             if (elect_one_sync()) {
                                 if (has_next) {
-                                    issue_qk(x, kaddr);
+                                    issue_qk(x, kaddr, kEarlyB ? 0 : 2);
                                     umma_commit(s_full(x));
                                 } else {
                                     umma_commit(o_full(x));
@@ -490,7 +498,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             tmem_wait_ld();
             // inside a run of skipped tiles the MMA warp issues S_x(j+1) as soon as S_x(j) has left TMEM
             const bool spec = kSparse && prev_skip && (j + 1) < T_c;
-            if (kSparse && !(DSA_EXP & 1)) {
+            if (kSparse || DSA_EARLY_B) {                    // S_x(j) has left TMEM
                 tc_fence_before();
                 if (lane == 0) mbar_arrive(s_read(x));
             }
@@ -642,6 +650,34 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 }
                 TRACE(16 + w)
                 const float neg_m = -m_used;
+#if DSA_F32X2
+                // x = s * scale - m for two logits per FFMA2, row sums as one packed pair per FADD2
+                const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
+                const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
+                uint64_t rs2 = pack_f32x2(0.f, 0.f);
+#pragma unroll
+                for (int c = 0; c < BC / 32; ++c) {          // 32 columns -> 16 packed bf16x2 -> P columns [16c, 16c+16)
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) {
+                        float x0, x1;
+                        unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(su[c][2 * i]), __uint_as_float(su[c][2 * i + 1])),
+                                               scale2, negm2), x0, x1);
+                        const float p0 = fast_exp2(x0);
+                        const float p1 = fast_exp2(x1);
+                        rs2 = add_f32x2(rs2, pack_f32x2(p0, p1));
+                        pk[i] = pack_bf16x2(p0, p1);
+                    }
+                    tmem_st_x16(tS + c * 16, pk);
+                    if (c == BC / 64 - 1) {                  // first half of P_X is in TMEM: its P V MMAs may start
+                        tmem_wait_st();
+                        tc_fence_before();
+                        mbar_arrive(p_half(x));
+                        TRACE(20 + w)
+                    }
+                }
+                unpack_f32x2(rs2, rs0, rs1);
+#else
 #pragma unroll
                 for (int c = 0; c < BC / 32; ++c) {          // 32 columns -> 16 packed bf16x2 -> P columns [16c, 16c+16)
                     uint32_t pk[16];
@@ -649,10 +685,8 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     for (int i = 0; i < 16; ++i) {
                         const float x0 = fmaf(__uint_as_float(su[c][2 * i]), scale_log2, neg_m);
                         const float x1 = fmaf(__uint_as_float(su[c][2 * i + 1]), scale_log2, neg_m);
-                        const bool emul = kEmulPairs >= 8 ? ((i & 1) == 1 && (i >> 1) < kEmulPairs)
-                                                          : ((i & 3) == 3 && (i >> 2) < kEmulPairs);
-                        const float p0 = emul ? exp2_fma(x0) : fast_exp2(x0);
-                        const float p1 = emul ? exp2_fma(x1) : fast_exp2(x1);
+                        const float p0 = fast_exp2(x0);
+                        const float p1 = fast_exp2(x1);
                         rs0 += p0;
                         rs1 += p1;
                         pk[i] = pack_bf16x2(p0, p1);
@@ -665,6 +699,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         TRACE(20 + w)
                     }
                 }
+#endif
                 if (kUseExpLock && nX == 2) st_shared_u32(sbase + L::kLockOff + 4 * (x * 4 + w), 0u);
             }
 #undef S_AT

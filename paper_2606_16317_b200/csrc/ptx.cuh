@@ -234,18 +234,25 @@ __device__ __forceinline__ float fast_exp2(float x) {
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// 2^x on the FMA / ALU pipes (no MUFU): x = n + f with n = round(x), f in [-0.5, 0.5];
-// 2^f by a degree-3 minimax polynomial (max relative error 7.5e-5, below bf16's 2^-9 rounding of P),
-// n added into the exponent field.  Used for a fraction of the softmax exponentials so that the
-// MUFU pipe (16 ex2/clk/SM) is not the only unit they queue on.  Requires x <= 126.
-__device__ __forceinline__ float exp2_fma(float x) {
-    x = fmaxf(x, -125.f);
-    const float t = x + 12582912.f;                   // 1.5 * 2^23: the low mantissa bits now hold round(x)
-    const float f = x - (t - 12582912.f);
-    float p = fmaf(0.0551716685f, f, 0.2426111251f);
-    p = fmaf(p, f, 0.6932609677f);
-    p = fmaf(p, f, 0.9999280572f);
-    return __int_as_float(__float_as_int(p) + (__float_as_int(t) << 23));
+// Packed pairs of fp32 on the FMA pipe (sm_100: fma / add .f32x2 take 64-bit register pairs): one issue slot for two
+// logits.  The softmax warps are bound by issue slots per exponential, not by any one pipe.
+__device__ __forceinline__ uint64_t pack_f32x2(float lo, float hi) {
+    uint64_t v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi));
+    return v;
+}
+__device__ __forceinline__ void unpack_f32x2(uint64_t v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t fma_f32x2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ uint64_t add_f32x2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
 }
 __device__ __forceinline__ float fast_log2(float x) {
     float y;
