@@ -63,9 +63,13 @@ constexpr int kMmaWarp1 = 11;
 // setmaxnreg: the kernel launches with 168 registers/thread (65536 / 384); the two softmax warpgroups grow to
 // 208 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 88.  The registers the 128
 // threads give up must cover what the 256 softmax threads take, or setmaxnreg.inc never returns.
+#ifndef DSA_REGS_SOFTMAX
+#define DSA_REGS_SOFTMAX 208
+#define DSA_REGS_OTHER 88
+#endif
 constexpr int kRegsLaunch = 168;
-constexpr int kRegsSoftmax = 208;
-constexpr int kRegsOther = 88;
+constexpr int kRegsSoftmax = DSA_REGS_SOFTMAX;
+constexpr int kRegsOther = DSA_REGS_OTHER;
 static_assert((kRegsLaunch - kRegsOther) * 128 >= (kRegsSoftmax - kRegsLaunch) * 256, "setmaxnreg pool imbalance");
 constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
