@@ -105,6 +105,39 @@ double sparse_attn_lambda_from_recall(double recall, int N);
 /* lambda = ln(p_real) + ln(tile_k / N)  (Eq. 7).  Pure host function. */
 double sparse_attn_lambda_from_preal(double p_real, int tile_k, int N);
 
+/*
+ * Spatio-temporal token re-ordering around the kernel (last sentence: "mapping the one-dimensional
+ * sequence back to its original spatiotemporal dimensions before processing ... can enhance the correlation within
+ * tiles"; PAPER.md:25 names the technique).  Tokens of a [grid_t, grid_h, grid_w] latent grid, stored in
+ * [t, h, w] order (n = (t * grid_h + h) * grid_w + w), are regrouped into bricks of brick_t x brick_h x brick_w
+ * cells so that 128 consecutive tokens are neighbours in time and space.
+ *
+ * sparse_attn_brick_permutation: pure host function.  Writes perm_out[p] = n, the original index of the token at
+ * position p of the brick order: bricks are visited in (t, h, w) order of their origin, the cells of a brick in
+ * (t, h, w) order; bricks at the upper edges of the grid are clipped to it (no padding), so perm_out is a
+ * permutation of 0 .. N-1 with N = grid_t * grid_h * grid_w.  perm_out is HOST memory, N int32, caller-owned.
+ * Errors: NULL pointer, any dimension <= 0, or N > 2^24 (SPARSE_ATTN_ERR_SHAPE).
+ */
+int sparse_attn_brick_permutation(int grid_t, int grid_h, int grid_w, int brick_t, int brick_h, int brick_w,
+                                  int32_t* perm_out);
+
+/*
+ * sparse_attn_reorder_tokens: gathers (inverse = 0) or scatters (inverse = 1) the token rows of a bf16 [B, H, N, D]
+ * tensor on the device:
+ *     inverse = 0:  dst[b, h, p, :]       = src[b, h, perm[p], :]     (into brick order, before the attention call)
+ *     inverse = 1:  dst[b, h, perm[p], :] = src[b, h, p, :]           (back to [t, h, w] order, on the output)
+ * src, dst: DEVICE, contiguous, 16-byte aligned, must not overlap; perm: DEVICE, N int32, a permutation of 0 .. N-1.
+ * Row-wise attention is permutation-equivariant: running sparse_attn_fwd on re-ordered q, k, v and scattering `out`
+ * back gives, in DENSE mode, the result of the un-permuted call up to summation order; in the sparse modes the
+ * decisions are taken on the re-ordered tiles (that is the point).  HBM-bound: 2 * B*H*N*D*2 bytes per call.
+ * Enqueues one kernel on `stream` (cudaStream_t, NULL = default stream) and returns; no host synchronisation.
+ * The entries of perm are NOT validated on the device (an out-of-range entry is undefined behaviour, as for any
+ * index array handed to a gather); sparse_attn_brick_permutation always produces a valid one.
+ * Errors: NULL pointers, bad shape, D not in {64, 128}, misaligned or overlapping buffers, no sm_100 device.
+ */
+int sparse_attn_reorder_tokens(const void* src, void* dst, int B, int H, int N, int D, const int32_t* perm,
+                               int inverse, void* stream);
+
 /* Static string for a status code. */
 const char* sparse_attn_status_string(int status);
 
@@ -114,7 +147,8 @@ const char* sparse_attn_last_error(void);
 /* SPARSE_ATTN_VERSION of the loaded library. */
 int sparse_attn_version(void);
 
-/* Number of kernel launches sparse_attn_fwd has enqueued in this process (for bench accounting). */
+/* Number of kernel launches sparse_attn_fwd and sparse_attn_reorder_tokens have enqueued in this process
+ * (for bench accounting). */
 int64_t sparse_attn_launch_count(void);
 
 #ifdef __cplusplus

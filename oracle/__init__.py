@@ -16,3 +16,4 @@ from .oracle import (  # noqa: F401
     run_head,
 )
 from .brute_force import brute_force_head  # noqa: F401
+from .reorder import brick_permutation, reorder  # noqa: F401

@@ -16,8 +16,10 @@ from .binding import (  # noqa: F401
     launch_count,
     library_path,
     make_params,
+    sparse_attn_brick_permutation,
     sparse_attn_fwd,
     sparse_attn_fwd_host,
+    sparse_attn_reorder_tokens,
     status_string,
     version,
 )

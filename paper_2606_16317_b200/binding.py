@@ -23,6 +23,8 @@ EXPORTED_SYMBOLS = (
     "sparse_attn_fwd_host",
     "sparse_attn_lambda_from_recall",
     "sparse_attn_lambda_from_preal",
+    "sparse_attn_brick_permutation",
+    "sparse_attn_reorder_tokens",
     "sparse_attn_status_string",
     "sparse_attn_last_error",
     "sparse_attn_version",
@@ -73,6 +75,11 @@ def _load():
         lib.sparse_attn_lambda_from_recall.argtypes = [ctypes.c_double, ctypes.c_int]
         lib.sparse_attn_lambda_from_preal.restype = ctypes.c_double
         lib.sparse_attn_lambda_from_preal.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int]
+        lib.sparse_attn_brick_permutation.restype = ctypes.c_int
+        lib.sparse_attn_brick_permutation.argtypes = [ctypes.c_int] * 6 + [ctypes.c_void_p]
+        lib.sparse_attn_reorder_tokens.restype = ctypes.c_int
+        lib.sparse_attn_reorder_tokens.argtypes = [ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 4 + [
+            ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
         lib.sparse_attn_status_string.restype = ctypes.c_char_p
         lib.sparse_attn_status_string.argtypes = [ctypes.c_int]
         lib.sparse_attn_last_error.restype = ctypes.c_char_p
@@ -154,3 +161,21 @@ def sparse_attn_fwd(q, k, v, out, lse, B, H, N, D, threshold_params, mode, stats
 def sparse_attn_fwd_host(q, k, v, out, lse, B, H, N, D, threshold_params, mode, stats_out):
     """C entry point `sparse_attn_fwd_host` (host buffers; copies inside, synchronous)."""
     return _call(_load().sparse_attn_fwd_host, q, k, v, out, lse, B, H, N, D, threshold_params, mode, stats_out)
+
+
+def sparse_attn_brick_permutation(grid_t, grid_h, grid_w, brick_t, brick_h, brick_w, perm_out):
+    """C entry point `sparse_attn_brick_permutation` (pure host function; perm_out: host int32 [N], numpy or address)."""
+    rc = _load().sparse_attn_brick_permutation(int(grid_t), int(grid_h), int(grid_w), int(brick_t), int(brick_h),
+                                               int(brick_w), _ptr(perm_out))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_reorder_tokens(src, dst, B, H, N, D, perm, inverse, stream=None):
+    """C entry point `sparse_attn_reorder_tokens` (device buffers; perm: device int32 [N])."""
+    rc = _load().sparse_attn_reorder_tokens(_ptr(src), _ptr(dst), int(B), int(H), int(N), int(D), _ptr(perm),
+                                            int(inverse), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc

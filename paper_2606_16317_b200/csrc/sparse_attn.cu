@@ -2,6 +2,7 @@
 // TMA tensor maps, launch.  No CPU fallback: without an sm_100 device every compute call fails.
 #include "../../include/sparse_attn.h"
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdarg>
@@ -10,6 +11,7 @@
 #include <cstring>
 
 #include "fwd_kernel.cuh"
+#include "reorder_kernel.cuh"
 
 // K / V ring depths of the D = 128 kernels (Q 64 KB + (NK + NV) x 32 KB must fit in 227 KB)
 #ifndef DSA_NK
@@ -23,6 +25,7 @@ namespace {
 
 thread_local char g_last_error[512] = "";
 std::atomic<int64_t> g_launches{0};
+std::atomic<int64_t> g_reorder_launches{0};
 
 int fail(int code, const char* fmt, ...) {
     va_list ap;
@@ -260,6 +263,58 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     return 0;
 }
 
+int sparse_attn_brick_permutation(int grid_t, int grid_h, int grid_w, int brick_t, int brick_h, int brick_w,
+                                  int32_t* perm_out) {
+    g_last_error[0] = '\0';
+    if (!perm_out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "perm_out must not be NULL");
+    if (grid_t <= 0 || grid_h <= 0 || grid_w <= 0 || brick_t <= 0 || brick_h <= 0 || brick_w <= 0)
+        return fail(SPARSE_ATTN_ERR_SHAPE, "grid and brick dimensions must be positive");
+    const long long N = static_cast<long long>(grid_t) * grid_h * grid_w;
+    if (N > (1 << 24)) return fail(SPARSE_ATTN_ERR_SHAPE, "N = %lld exceeds 2^24", N);
+    int32_t* p = perm_out;
+    for (int t0 = 0; t0 < grid_t; t0 += brick_t)
+        for (int h0 = 0; h0 < grid_h; h0 += brick_h)
+            for (int w0 = 0; w0 < grid_w; w0 += brick_w)
+                for (int t = t0; t < t0 + brick_t && t < grid_t; ++t)
+                    for (int h = h0; h < h0 + brick_h && h < grid_h; ++h)
+                        for (int w = w0; w < w0 + brick_w && w < grid_w; ++w)
+                            *p++ = (t * grid_h + h) * grid_w + w;
+    return 0;
+}
+
+int sparse_attn_reorder_tokens(const void* src, void* dst, int B, int H, int N, int D, const int32_t* perm,
+                               int inverse, void* stream) {
+    g_last_error[0] = '\0';
+    if (!src || !dst || !perm) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "src, dst and perm must not be NULL");
+    if (B <= 0 || H <= 0 || N <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N must be positive (got %d, %d, %d)", B, H, N);
+    if (N > (1 << 24)) return fail(SPARSE_ATTN_ERR_SHAPE, "N = %d exceeds 2^24", N);
+    if (D != 64 && D != 128) return fail(SPARSE_ATTN_ERR_HEAD_DIM, "D = %d not in {64, 128}", D);
+    const size_t bytes = static_cast<size_t>(B) * H * N * D * 2;
+    const uintptr_t s0 = reinterpret_cast<uintptr_t>(src), d0 = reinterpret_cast<uintptr_t>(dst);
+    if ((s0 | d0) & 15u) return fail(SPARSE_ATTN_ERR_ALIGNMENT, "src and dst must be 16-byte aligned");
+    if (s0 < d0 + bytes && d0 < s0 + bytes) return fail(SPARSE_ATTN_ERR_PARAMS, "src and dst overlap");
+    int rc = check_device();
+    if (rc) return rc;
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        CUDA_TRY(cudaGetDevice(&dev));
+        CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    const long long rows = static_cast<long long>(B) * H * N;
+    const int lanes = D / 8;                                 // 16 bytes per thread
+    const long long blocks_needed = (rows + (256 / lanes) * 4 - 1) / ((256 / lanes) * 4);
+    const int grid = static_cast<int>(std::min<long long>(blocks_needed, static_cast<long long>(n_sm) * 8));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (lanes == 16)
+        dsa::reorder_tokens_kernel<16><<<grid, 256, 0, st>>>(static_cast<const uint4*>(src), static_cast<uint4*>(dst), perm, rows, N, inverse ? 1 : 0);
+    else
+        dsa::reorder_tokens_kernel<8><<<grid, 256, 0, st>>>(static_cast<const uint4*>(src), static_cast<uint4*>(dst), perm, rows, N, inverse ? 1 : 0);
+    CUDA_TRY(cudaGetLastError());
+    g_reorder_launches.fetch_add(1);
+    return 0;
+}
+
 double sparse_attn_lambda_from_recall(double recall, int N) { return std::log((1.0 - recall) / N); }
 
 double sparse_attn_lambda_from_preal(double p_real, int tile_k, int N) {
@@ -286,6 +341,6 @@ const char* sparse_attn_last_error(void) { return g_last_error; }
 
 int sparse_attn_version(void) { return SPARSE_ATTN_VERSION; }
 
-int64_t sparse_attn_launch_count(void) { return g_launches.load(); }
+int64_t sparse_attn_launch_count(void) { return g_launches.load() + g_reorder_launches.load(); }
 
 }  // extern "C"
