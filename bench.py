@@ -32,6 +32,7 @@ from workloads import CONFIGS, make_qkv  # noqa: E402
 METRIC = "attention ms & effective TFLOP/s vs dense mode at Wan-2.2 shapes; sparsity %; % tensor peak"
 P_REAL = 1.5            # Eq. 7 "transition region" constant
 FALLBACK_TFLOPS = 1590.0
+BRICK = (4, 4, 8)       # token re-ordering brick (t, h, w): 128 tokens = one attention tile
 # dram__bytes_read.sum + dram__bytes_write.sum of one DENSE config-1 launch, ncu --set full (profiles/ncu_dense_r01.md);
 # algorithmic bytes: q + k + v + out + lse = 4 * 201.3 MB + 3.1 MB = 808 MB
 NCU_DRAM_BYTES_DENSE_CFG1 = 608.95e6 + 188.01e6
@@ -67,17 +68,22 @@ class ClockSampler:
 
     def __init__(self, index=0):
         self.samples, self._stop, self.index = [], threading.Event(), index
+        self.active = threading.Event()         # set only while a timed region runs: idle gaps are not sampled
         self._t = threading.Thread(target=self._run, daemon=True)
 
     def _run(self):
         while not self._stop.is_set():
+            if not self.active.is_set():
+                self._stop.wait(0.005)
+                continue
             try:
                 out = subprocess.run(["nvidia-smi", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
                                       "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
-                self.samples.append([s.strip() for s in out.strip().split(",")])
+                if self.active.is_set():         # the region was still running when nvidia-smi returned
+                    self.samples.append([s.strip() for s in out.strip().split(",")])
             except Exception:
                 pass
-            self._stop.wait(0.1)
+            self._stop.wait(0.02)
 
     def __enter__(self):
         self._t.start()
@@ -152,7 +158,7 @@ def workload_name(cfg):
 
 
 # ---------------------------------------------------------------------------------------------- GPU arm
-def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier):
+def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier, sampler=None):
     """Returns (total_ms over `steps` calls, per-call ms list, stats [B,H,2])."""
     q, k, v, out, lse, stats = bufs
     stream = torch.cuda.current_stream()
@@ -162,14 +168,61 @@ def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier):
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
     barrier()
     torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.active.set()
     evs[0].record(stream)
     for i in range(steps):
         sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p, mode, stats)
         evs[i + 1].record(stream)
     torch.cuda.synchronize()
+    if sampler is not None:
+        sampler.active.clear()
     barrier()
     per = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
     return evs[0].elapsed_time(evs[-1]), per, stats.cpu().numpy().copy()
+
+
+def time_reorder(sa, torch, cfg, brick, qkv, scratch_out, steps, warmup):
+    """Re-orders q, k, v into brick order with sparse_attn_reorder_tokens and times the four passes a call needs
+    (three gathers before the attention, one scatter of `out` after it)."""
+    perm = np.empty(cfg.N, dtype=np.int32)
+    sa.sparse_attn_brick_permutation(*cfg.grid, *brick, perm)
+    dperm = torch.from_numpy(perm).cuda()
+    stream = torch.cuda.current_stream()
+    dst = [torch.empty_like(t) for t in qkv]
+    back = torch.empty_like(scratch_out)
+
+    def four_passes():
+        for s_, d_ in zip(qkv, dst):
+            sa.sparse_attn_reorder_tokens(s_, d_, cfg.B, cfg.H, cfg.N, cfg.D, dperm, 0, stream.cuda_stream)
+        sa.sparse_attn_reorder_tokens(dst[0], back, cfg.B, cfg.H, cfg.N, cfg.D, dperm, 1, stream.cuda_stream)
+
+    for _ in range(max(warmup, 1)):
+        four_passes()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        four_passes()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    assert torch.equal(back, qkv[0]), "gather followed by scatter must give the input back"
+    ms = e0.elapsed_time(e1) / steps
+    nbytes = 4 * 2 * qkv[0].numel() * 2                     # 4 passes, each reads and writes the tensor once
+    hbm = measured_hbm()
+    info = {"brick": list(brick), "ms_4_passes": ms, "bytes_4_passes": nbytes, "achieved_gbs": nbytes / (ms * 1e-3) / 1e9,
+            "hbm_peak_gbs": hbm, "frac_of_hbm_peak": nbytes / (ms * 1e-3) / 1e9 / hbm,
+            "note": "3 gathers (q, k, v) + 1 scatter (out) per attention call; 805 MB read + 805 MB written > L2"}
+    del back
+    return info, tuple(dst)
+
+
+def measured_hbm():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"])
+    return 6650.0                                           # fallback stated in B200_PROFILING.md
 
 
 def main():
@@ -218,19 +271,30 @@ def main():
         return torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
 
     results = {}
-    variants = [args.config] + ([] if args.no_aligned or args.config + "_aligned" not in CONFIGS
-                                else [args.config + "_aligned"])
+    # (result key, generator config, brick of the token re-ordering or None)
+    variants = [(args.config, args.config, None)]
+    if not args.no_aligned:
+        if args.config + "_aligned" in CONFIGS:
+            variants.append((args.config + "_aligned", args.config + "_aligned", None))
+        # SURVEY.md 8(f) NEXT-1 / PAPER.md:139: the contract workload with its tokens re-ordered into bricks
+        variants.append((args.config + "_brick%dx%dx%d" % BRICK, args.config, BRICK))
+    reorder_info = None
     head_total_ms = None
     sampler = ClockSampler(local_rank)
-    sampler.__enter__()                     # clocks / throttle reasons are sampled across every timed region below
+    sampler.__enter__()                     # clocks / throttle reasons are sampled inside every timed region below
     launches0 = sa.launch_count()
     headline_launches = 0
-    for vi, name in enumerate(variants):
-        vcfg = CONFIGS[name]
+    for vi, (name, gen_name, brick) in enumerate(variants):
+        vcfg = CONFIGS[gen_name]
         # weak scaling: every rank draws its own batch (different seed), same shape
-        qb, kb, vb = make_qkv(vcfg, args.seed + 1000 * rank)
+        if brick is None or gen_name != variants[0][1]:
+            qb, kb, vb = make_qkv(vcfg, args.seed + 1000 * rank)
+        else:
+            qb, kb, vb = keep_bufs                       # same bits as the contract workload
         q, k, v = to_dev(qb), to_dev(kb), to_dev(vb)
         out = torch.empty_like(q)
+        if brick is not None:
+            reorder_info, (q, k, v) = time_reorder(sa, torch, vcfg, brick, (q, k, v), out, args.steps, args.warmup)
         lse = torch.empty((cfg.B, cfg.H, cfg.N), device="cuda", dtype=torch.float32)
         stats = torch.zeros((cfg.B, cfg.H, 2), device="cuda", dtype=torch.int64)
         bufs = (q, k, v, out, lse, stats)
@@ -242,11 +306,11 @@ def main():
             headline = (vi == 0 and mname == "dynamic")
             if headline:
                 l0 = sa.launch_count()
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier)
+                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler)
                 headline_launches = sa.launch_count() - l0 - args.warmup
                 head_total_ms = total
             else:
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier)
+                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler)
             if dist is not None:
                 t = torch.tensor([total], device="cuda")
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -258,6 +322,16 @@ def main():
                 st_all = st[None]
             ms = total / args.steps
             ex = executed_flop(BH * world, cfg.N, cfg.D, cfg.tile, st_all)
+            if mname == "dense":
+                out_dense, lse_dense = out.clone(), lse.clone()
+                quality = {}
+            elif "dense" in res:
+                # achieved recall per row = exp(lse_retained - lse_dense), error against dense
+                rec = torch.exp(lse - lse_dense)
+                err = (out.float() - out_dense.float()).abs()
+                quality = {"recall_min": float(rec.min()), "recall_mean": float(rec.mean()),
+                           "err_vs_dense_max_abs": float(err.max()), "err_vs_dense_mean_abs": float(err.mean())}
+                del rec, err
             res[mname] = {
                 "ms": ms, "ms_min": float(np.min(per)), "ms_median": float(np.median(per)),
                 "sparsity": float(st_all[..., 1].sum() / st_all.sum()),
@@ -265,15 +339,24 @@ def main():
                 "executed_tflops": ex / (ms * 1e-3) / 1e12,
                 "kernel_ms_avg_rank0": float(np.mean(per)),
                 "executed_flop_per_launch_rank0": executed_flop(BH, cfg.N, cfg.D, cfg.tile, st[None]),
+                **quality,
             }
         for mname in ("fixed", "dynamic"):
             if mname not in res or "dense" not in res:
                 continue
             res[mname]["speedup_vs_dense"] = res["dense"]["ms"] / res[mname]["ms"]
             res[mname]["mma_bound_model"] = 1.0 / (1.0 - res[mname]["sparsity"] / 2.0)
+        if brick is not None and reorder_info is not None:
+            for mname in ("fixed", "dynamic"):
+                if mname in res and "dense" in results.get(variants[0][0], {}):
+                    # whole re-ordered pipeline (3 gathers + attention + 1 scatter) against the plain DENSE call
+                    res[mname]["ms_with_reorder"] = res[mname]["ms"] + reorder_info["ms_4_passes"]
+                    res[mname]["speedup_vs_plain_dense_incl_reorder"] = (
+                        results[variants[0][0]]["dense"]["ms"] / res[mname]["ms_with_reorder"])
         results[name] = res
         if vi == 0:
             keep_bufs = (qb, kb, vb)
+        out_dense = lse_dense = None
         del q, k, v, out, lse, stats, bufs
         torch.cuda.empty_cache()
 
@@ -350,6 +433,7 @@ def main():
         "e2e": {"value": dense_flop(BH * world, cfg.N, cfg.D) / e2e_s / 1e12,
                 "unit": "TFLOP/s (dense-equivalent, host buffers, H2D + kernel + D2H)",
                 "ms_per_step": e2e_s * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "token_reordering": reorder_info,
         "gpu_launches": headline_launches,
         "clocks": clocks,
     }
