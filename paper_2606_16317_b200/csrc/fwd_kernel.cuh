@@ -189,7 +189,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     volatile int* votes = reinterpret_cast<volatile int*>(smem + L::kVotesOff);                  // [2][4][4]
     volatile float* wmax = reinterpret_cast<volatile float*>(smem + L::kVotesOff + 128);         // [2][4][4]
 
-    const int warp = threadIdx.x >> 5;
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform: role and slot indices live in uniform registers
     const int lane = threadIdx.x & 31;
     const int bh = blockIdx.y;
     const int tile0 = blockIdx.x * 2;
