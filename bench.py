@@ -212,7 +212,8 @@ def time_reorder(sa, torch, cfg, brick, qkv, scratch_out, steps, warmup):
     hbm = measured_hbm()
     info = {"brick": list(brick), "ms_4_passes": ms, "bytes_4_passes": nbytes, "achieved_gbs": nbytes / (ms * 1e-3) / 1e9,
             "hbm_peak_gbs": hbm, "frac_of_hbm_peak": nbytes / (ms * 1e-3) / 1e9 / hbm,
-            "note": "3 gathers (q, k, v) + 1 scatter (out) per attention call; 805 MB read + 805 MB written > L2"}
+            "note": "3 gathers (q, k, v) + 1 scatter (out) per attention call; %.0f MB read + %.0f MB written, larger than L2"
+                    % (nbytes / 2e6, nbytes / 2e6)}
     del back
     return info, tuple(dst)
 
