@@ -36,7 +36,7 @@ enum sparse_attn_status {
     SPARSE_ATTN_ERR_NULL_POINTER = -1, /* a required pointer is NULL */
     SPARSE_ATTN_ERR_SHAPE = -2,        /* B, H or N <= 0, or B*H / N too large for the launch */
     SPARSE_ATTN_ERR_HEAD_DIM = -3,     /* D not in {64, 128} */
-    SPARSE_ATTN_ERR_TILE = -4,         /* tile_q / tile_k not the supported decision tile for this D */
+    SPARSE_ATTN_ERR_TILE = -4,         /* tile_q / tile_k not a supported decision tile for this D and mode */
     SPARSE_ATTN_ERR_MODE = -5,         /* mode not in {0, 1, 2} */
     SPARSE_ATTN_ERR_PARAMS = -6,       /* params NULL in a sparse mode, struct_size wrong, lambda NaN,
                                           lambda > 0 in FIXED mode, softmax_scale negative / non-finite */
@@ -55,7 +55,11 @@ typedef struct sparse_attn_params {
                                -INFINITY disables skipping.  In FIXED mode it is ln(alpha) and must be <= 0. */
     float softmax_scale;    /* 0 means 1/sqrt(D) */
     int32_t tile_q;         /* decision tile rows B_r; 0 = default (64 for D = 64, 128 for D = 128) */
-    int32_t tile_k;         /* decision tile columns B_c; 0 = default (same as tile_q) */
+    int32_t tile_k;         /* decision tile columns B_c; 0 = default (same as tile_q).
+                               D = 128 also accepts tile_q = 128 with tile_k = 64 or 32 in the sparse modes ("block
+                               size 32"): the decision tiles of 64 / 32 keys are visited in ascending
+                               key order, the statistics are updated after every retained one, and exp, row sum and
+                               P V are skipped per decision tile.  T_c below is then ceil(N / tile_k). */
     void* stream;           /* cudaStream_t to launch on; NULL = the default stream */
     uint8_t* skip_mask_out; /* optional, device, [B, H, T_r, T_c] bytes, 1 = tile skipped, fully overwritten.
                                T_r = ceil(N / tile_q), T_c = ceil(N / tile_k).  NULL in timed runs. */

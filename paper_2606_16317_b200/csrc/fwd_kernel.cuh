@@ -106,11 +106,12 @@ struct FwdArgs {
     __nv_bfloat16* out;          // [BH, N, D]
     float* lse;                  // [BH, N] or null
     unsigned long long* stats;   // [BH, 2] or null (pre-zeroed)
-    uint8_t* skip_mask;          // [BH, T_r, T_c] or null
-    float* margin;               // [BH, T_r, T_c] or null
+    uint8_t* skip_mask;          // [BH, T_r, T_c_dec] or null
+    float* margin;               // [BH, T_r, T_c_dec] or null
     int N;
     int T_r;                     // decision tiles along queries
-    int T_c;                     // decision tiles along keys (= K tiles)
+    int T_c;                     // K tiles of BC keys (MMA tiles)
+    int T_c_dec;                 // decision tiles along keys: ceil(N / tile_k), = T_c unless tile_k < BC
     int n_mma_tiles;             // ceil(N / 128)
     int mode;
     float scale_log2;            // softmax_scale * log2(e)
@@ -134,11 +135,12 @@ struct SmemLayout {
     //                      s_full[2] p_half[2] p_ready[2] o_full[2] s_read[2] dec[2][4]
     static constexpr int kNumBars = 2 + 2 * NK + 2 * NV + 8 + 2 + 8;
     static constexpr int kMiscOff = kBarOff + 8 * kNumBars;
-    // misc: tmem_ptr (4) | pad (12) | votes[2][4][4] (128) | wmax[2][4][4] (128) | in_exp[2][4] (32) | prog[2] (16)
+    // misc: tmem_ptr (4) | pad (12) | votes[2][4][4] (128) | wmax[2][4][4] (128) | in_exp[2][4] (32) | prog[2] (16) | pvmask[2][4] (32)
     static constexpr int kVotesOff = kMiscOff + 16;
     static constexpr int kLockOff = kVotesOff + 256;
     static constexpr int kProgOff = kLockOff + 32;
-    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16;
+    static constexpr int kPvMaskOff = kProgOff + 16;       // pvmask[2][4]: kept sub-tiles of tile j (SUB > 1), ring like votes
+    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16 + 32;
     static constexpr int kTotal = kMiscOff + kMiscBytes;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
     static_assert(kDynamicBytes <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
@@ -146,7 +148,9 @@ struct SmemLayout {
 
 // kSparse = false compiles the DENSE mode only (no predicate, no vote, V always fetched);
 // kDebug adds the optional skip_mask_out / margin_out parity outputs.
-template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug>
+// SUB > 1 (sparse modes, G = 1): the decision tile is BR x (BC / SUB) keys -- SUB decisions per MMA tile, taken in
+// ascending key order with the statistics updated after every retained one (block size 32).
+template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug, int SUB = 1>
 __global__ void __launch_bounds__(kNumThreads, 1)
 sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
                        const __grid_constant__ CUtensorMap tm_v, const FwdArgs a) {
@@ -154,6 +158,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     static_assert(D == 64 || D == 128, "head dim");
     static_assert(BC == 64 || BC == 128, "key tile");
     static_assert(2 * BC + 2 * D <= kTmemCols, "TMEM budget");
+    static_assert(SUB == 1 || (kSparse && G == 1 && (SUB == 2 || SUB == 4) && (BC / SUB) % 32 == 0), "sub-tile decisions");
     constexpr int BR = 128 / G;
     constexpr int kSubD = D / 64;
     constexpr uint32_t kIdescQK = umma_idesc_bf16(128, BC, 0);   // S = Q K^T: A, B both K-major
@@ -328,9 +333,11 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             umma_smem_desc_sw128(kaddr + koff, 16, 1024), h == 2 ? kIdescQK : kIdescQKh, kk > 0);
                 }
             };
-            auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int half) {   // half 0 / 1: keys [0, BC/2) / [BC/2, BC)
+            // half 0 / 1: keys [0, BC/2) / [BC/2, BC); mask (SUB > 1): bit s set = decision sub-tile s was kept
+            auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int half, uint32_t mask = 0xffu) {
 #pragma unroll
                 for (int kk = half * (BC / 32); kk < (half + 1) * (BC / 32); ++kk) {
+                    if (SUB > 1 && !((mask >> (kk / (BC / 16 / SUB))) & 1u)) continue;   // P of a skipped sub-tile is never read
                     // 16 keys = 16 rows of 128 B; d sub-tiles (64 columns) are L::kSubKVBytes apart (LBO)
                     umma_ts(tmem_base + 2 * BC + x * D, tmem_base + x * BC + kk * 8,
                             umma_smem_desc_sw128(vaddr + kk * 2048, L::kSubKVBytes, 1024), kIdescPV, acc || kk > 0);
@@ -409,14 +416,16 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         mbar_wait(p_half(x), ppar[x]);
                         mbar_wait(v_full(vslot), vph);       // V_j has landed (sparse modes: fetched by the V warp
                         tc_fence_after();                    // once some slot voted to keep tile j, or prefetched)
-                        if (elect_one_sync()) issue_pv(x, vaddr, j > 0, 0);
+                        uint32_t pvmask = 0xffu;
+                        if (SUB > 1) pvmask = ld_shared_u32(sbase + L::kPvMaskOff + (x * 4 + (j & 3)) * 4);
+                        if (elect_one_sync()) issue_pv(x, vaddr, j > 0, 0, pvmask);
                         __syncwarp();
                         mbar_wait(p_ready(x), ppar[x]);
                         tc_fence_after();
                         ppar[x] ^= 1u;
                         TRACE(2)
                         if (elect_one_sync()) {
-                            issue_pv(x, vaddr, true, 1);
+                            issue_pv(x, vaddr, true, 1, pvmask);
                             umma_commit(v_empty(vslot));     // this slot's P_x V_j has read V_j
                             if (has_next) {
                                 issue_qk(x, kaddr, kEarlyB ? 0 : 2);   // (again, if a speculative one was overwritten by P_x)
@@ -468,7 +477,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         const int dtile = mma_tile * G + grp;
         const bool grp_valid = dtile < a.T_r;
         const bool grp_leader = (r % BR) == 0;
-        const size_t tile_row = (static_cast<size_t>(bh) * a.T_r + dtile) * static_cast<size_t>(T_c);
+        const size_t tile_row = (static_cast<size_t>(bh) * a.T_r + dtile) * static_cast<size_t>(a.T_c_dec);
         const int mode = a.mode;
         const float scale_log2 = a.scale_log2;
         const float lambda_log2 = a.lambda_log2;
@@ -529,6 +538,124 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             if (w == 0) { TRACE(7) }
             PROF_TICK(3)
 
+            if constexpr (SUB > 1) {
+                // ============ decision tiles of BC / SUB keys: SUB decisions per MMA tile, in key order
+                constexpr int W = BC / SUB;                  // keys per decision tile (32 or 64)
+                const int q = j & 3;
+                // the stabiliser m_used follows the max of the WHOLE MMA tile (it only has to bound the exponents; a
+                // sub-tile with a large max is never skipped), so it is fixed before any P of this tile is written
+                if (j == 0) {
+                    m_used = mhat2;
+                } else {
+                    const bool need = mhat2 > m_used + kRescaleThreshold;
+                    if (__any_sync(0xffffffffu, need)) {
+                        const float alpha = need ? fast_exp2(m_used - mhat2) : 1.f;
+                        if (need) m_used = mhat2;
+                        l *= alpha;                          // (m_used + log2 l, hence lse2, is unchanged)
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {   // O_r *= alpha (PV of tile j-1 has completed: s_full(j))
+                            uint32_t o[32];
+                            tmem_ld_x32(tO + c * 32, o);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                            tmem_st_x32(tO + c * 32, o);
+                        }
+                    }
+                }
+                const float neg_m = -m_used;
+                const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
+                const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
+                uint32_t kept = 0u;                          // bit s: decision sub-tile s retained
+#pragma unroll
+                for (int s = 0; s < SUB; ++s) {
+                    const int jj = j * SUB + s;              // decision tile index along the keys
+                    if (jj >= a.T_c_dec) break;              // beyond the last key (ragged tail): no such tile
+                    float ms = S_AT(s * W);
+#pragma unroll
+                    for (int c = 1; c < W; ++c) ms = fmaxf(ms, S_AT(s * W + c));
+                    ms *= scale_log2;                        // a3 for this decision tile
+                    const float ref = (mode == kModeDynamic) ? lse2 : m_true;
+                    const float t2 = ms - ref;               // Eq. 5, log2 units (+inf before the first retained tile)
+                    const bool row_skip = (jj > 0) && (!row_valid || (t2 < lambda_log2));
+                    const bool skip_s = named_bar_red_and(1 + x, 128, row_skip);   // all 128 rows of the Q tile (R1)
+                    if (kDebug) {
+                        float gm = INFINITY;
+                        if (want_margin) {
+                            float tm = row_valid ? t2 : -INFINITY;
+#pragma unroll
+                            for (int o = 16; o > 0; o >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, o));
+                            if (lane == 0) wmax[(x * 4 + q) * 4 + w] = tm;
+                            named_bar_sync(1 + x, 128);
+                            gm = fmaxf(fmaxf(wmax[(x * 4 + q) * 4 + 0], wmax[(x * 4 + q) * 4 + 1]),
+                                       fmaxf(wmax[(x * 4 + q) * 4 + 2], wmax[(x * 4 + q) * 4 + 3]));
+                            gm = (jj == 0) ? INFINITY : (gm - lambda_log2) * kLn2;
+                            named_bar_sync(1 + x, 128);
+                        }
+                        if (grp_leader && grp_valid) {
+                            if (a.skip_mask) a.skip_mask[tile_row + jj] = skip_s ? 1 : 0;
+                            if (want_margin) a.margin[tile_row + jj] = gm;
+                        }
+                    }
+                    if (skip_s) {
+                        if (grp_leader && grp_valid) ++n_skip;
+                        continue;                            // a7: this decision tile leaves m, l, O untouched
+                    }
+                    if (grp_leader && grp_valid) ++n_exec;
+                    if (kept == 0u) {
+                        // first retained sub-tile: the MMA tile is kept -- tell the issuer and the V warp now
+                        tc_fence_before();
+                        if (lane == 0) {
+                            votes[(x * 4 + q) * 4 + w] = (j << 2) | 2;
+                            mbar_arrive(dec(x, q));
+                        }
+                        __syncwarp();
+                        if (spec) {                          // a speculative S_x(j+1) is in flight over these columns
+                            mbar_wait(s_full(x), sfpar);
+                            sfpar ^= 1u;
+                            tc_fence_after();
+                        }
+                    }
+                    kept |= 1u << s;
+                    m_true = fmaxf(m_true, ms);
+                    uint64_t rs2 = pack_f32x2(0.f, 0.f);
+#pragma unroll
+                    for (int c = s * (W / 32); c < (s + 1) * (W / 32); ++c) {
+                        uint32_t pk[16];
+#pragma unroll
+                        for (int i = 0; i < 16; ++i) {
+                            float x0, x1;
+                            unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(su[c][2 * i]), __uint_as_float(su[c][2 * i + 1])),
+                                                   scale2, negm2), x0, x1);
+                            const float p0 = fast_exp2(x0);
+                            const float p1 = fast_exp2(x1);
+                            rs2 = add_f32x2(rs2, pack_f32x2(p0, p1));
+                            pk[i] = pack_bf16x2(p0, p1);
+                        }
+                        tmem_st_x16(tS + c * 16, pk);
+                    }
+                    float r0, r1;
+                    unpack_f32x2(rs2, r0, r1);
+                    l += r0 + r1;                            // the next decision of this tile needs the new LSE (Eq. 6)
+                    if (mode == kModeDynamic) lse2 = m_used + fast_log2(l);
+                }
+                prev_skip = kept == 0u;
+                if (kept == 0u) {                            // every sub-tile skipped: the MMA tile is skipped
+                    tc_fence_before();
+                    if (lane == 0) {
+                        votes[(x * 4 + q) * 4 + w] = (j << 2) | 1;
+                        mbar_arrive(dec(x, q));
+                    }
+                    __syncwarp();
+                    continue;
+                }
+                if (w == 0 && lane == 0) st_shared_u32(sbase + L::kPvMaskOff + (x * 4 + q) * 4, kept);
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(p_half(x));                      // (release: the mask above is visible to the issuer)
+                mbar_arrive(p_ready(x));
+                continue;
+            }
             // ---- predicate and all-rows vote (a4)
             bool skip_grp = false, keep_any = true;
             float grp_margin = INFINITY;

@@ -74,11 +74,11 @@ int make_tmap(EncodeTiledFn enc, CUtensorMap* tm, const void* base, int BH, int 
     return 0;
 }
 
-template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug>
+template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug, int SUB = 1>
 int launch(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, const dsa::FwdArgs& args, int BH,
            cudaStream_t stream) {
     using L = dsa::SmemLayout<D, BC, NK, NV>;
-    auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NK, NV, kSparse, kDebug>;
+    auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NK, NV, kSparse, kDebug, SUB>;
     static bool configured = false;
     if (!configured) {
         CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L::kDynamicBytes));
@@ -127,8 +127,12 @@ int validate(const void* q, const void* k, const void* v, void* out, int B, int 
             return fail(SPARSE_ATTN_ERR_PARAMS, "softmax_scale must be finite and >= 0 (0 = 1/sqrt(D))");
         const int tq = p->tile_q ? p->tile_q : def_tile;
         const int tk = p->tile_k ? p->tile_k : tq;
-        if (tq != def_tile || tk != def_tile)
-            return fail(SPARSE_ATTN_ERR_TILE, "decision tile %dx%d unsupported for D = %d (supported: %dx%d)", tq, tk, D, def_tile, def_tile);
+        // D = 128 also takes decision tiles of 128 x 64 and 128 x 32 keys (block size 32 for the 5B model)
+        const bool sub_ok = D == 128 && tq == 128 && (tk == 64 || tk == 32) && mode != SPARSE_ATTN_DENSE;
+        if ((tq != def_tile || tk != def_tile) && !sub_ok)
+            return fail(SPARSE_ATTN_ERR_TILE, "decision tile %dx%d unsupported for D = %d in mode %d (supported: %dx%d%s)", tq, tk, D,
+                        mode, def_tile, def_tile, D == 128 ? ", and 128x64 / 128x32 in the sparse modes" : "");
+        r->tile_k = tk;
         if (p->softmax_scale > 0.f) r->scale = p->softmax_scale;
         r->lambda = p->lambda;
         r->stream = static_cast<cudaStream_t>(p->stream);
@@ -171,8 +175,9 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     const int BH = B * H;
     CUtensorMap tq, tk, tv;
     if ((rc = make_tmap(enc, &tq, q, BH, N, D, 128))) return rc;
-    if ((rc = make_tmap(enc, &tk, k, BH, N, D, r.tile_k))) return rc;
-    if ((rc = make_tmap(enc, &tv, v, BH, N, D, r.tile_k))) return rc;
+    const int mma_k = (D == 64) ? 64 : 128;                 // keys per MMA tile (the decision tile may be narrower)
+    if ((rc = make_tmap(enc, &tk, k, BH, N, D, mma_k))) return rc;
+    if ((rc = make_tmap(enc, &tv, v, BH, N, D, mma_k))) return rc;
 
     dsa::FwdArgs a;
     a.out = static_cast<__nv_bfloat16*>(out);
@@ -182,7 +187,8 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     a.margin = r.margin;
     a.N = N;
     a.T_r = (N + r.tile_q - 1) / r.tile_q;
-    a.T_c = (N + r.tile_k - 1) / r.tile_k;
+    a.T_c = (N + mma_k - 1) / mma_k;
+    a.T_c_dec = (N + r.tile_k - 1) / r.tile_k;
     a.n_mma_tiles = (N + 127) / 128;
     a.mode = mode;
     a.scale_log2 = r.scale * dsa::kLog2e;
@@ -197,6 +203,14 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     if (D == 128) {
         if (!sparse && !debug) return launch<128, 128, 1, DSA_NK, DSA_NV, false, false>(tq, tk, tv, a, BH, r.stream);
         if (!sparse) return launch<128, 128, 1, DSA_NK, DSA_NV, false, true>(tq, tk, tv, a, BH, r.stream);
+        if (r.tile_k == 64) {
+            if (!debug) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false, 2>(tq, tk, tv, a, BH, r.stream);
+            return launch<128, 128, 1, DSA_NK, DSA_NV, true, true, 2>(tq, tk, tv, a, BH, r.stream);
+        }
+        if (r.tile_k == 32) {
+            if (!debug) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false, 4>(tq, tk, tv, a, BH, r.stream);
+            return launch<128, 128, 1, DSA_NK, DSA_NV, true, true, 4>(tq, tk, tv, a, BH, r.stream);
+        }
         if (!debug) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false>(tq, tk, tv, a, BH, r.stream);
         return launch<128, 128, 1, DSA_NK, DSA_NV, true, true>(tq, tk, tv, a, BH, r.stream);
     }

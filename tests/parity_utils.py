@@ -36,7 +36,7 @@ def to_dev_bf16(bits: np.ndarray) -> torch.Tensor:
 
 
 def run_gpu(q_bits: np.ndarray, k_bits: np.ndarray, v_bits: np.ndarray, *, mode: int, lam: float = -math.inf,
-            tile: int, debug: bool = True, scale: float = 0.0) -> GpuResult:
+            tile: int, debug: bool = True, scale: float = 0.0, tile_k: int = 0) -> GpuResult:
     """q/k/v bits: uint16 [B, H, N, D].  Calls the C ABI through the binding on cuda:0."""
     B, H, N, D = q_bits.shape
     q, k, v = (to_dev_bf16(np.ascontiguousarray(x)) for x in (q_bits, k_bits, v_bits))
@@ -44,16 +44,17 @@ def run_gpu(q_bits: np.ndarray, k_bits: np.ndarray, v_bits: np.ndarray, *, mode:
     lse = torch.full((B, H, N), float("nan"), device="cuda", dtype=torch.float32)
     stats = torch.full((B, H, 2), -1, device="cuda", dtype=torch.int64)
     T = -(-N // tile)
-    mask = torch.full((B, H, T, T), 255, device="cuda", dtype=torch.uint8) if debug else None
-    margin = torch.full((B, H, T, T), float("nan"), device="cuda", dtype=torch.float32) if debug else None
+    Tc = -(-N // (tile_k or tile))                     # decision tiles along the keys (tile_k < tile: SURVEY.md NEXT-2)
+    mask = torch.full((B, H, T, Tc), 255, device="cuda", dtype=torch.uint8) if debug else None
+    margin = torch.full((B, H, T, Tc), float("nan"), device="cuda", dtype=torch.float32) if debug else None
     p = sa.make_params(lam=lam, softmax_scale=scale, stream=torch.cuda.current_stream().cuda_stream,
-                       skip_mask_out=mask, margin_out=margin)
+                       skip_mask_out=mask, margin_out=margin, tile_q=tile if tile_k else 0, tile_k=tile_k)
     sa.sparse_attn_fwd(q, k, v, out, lse, B, H, N, D, p, mode, stats)
     torch.cuda.synchronize()
     out64 = bf16_bits_to_f64(out.view(torch.int16).cpu().numpy().view(np.uint16)).reshape(B * H, N, D)
     return GpuResult(out64, lse.cpu().numpy().reshape(B * H, N), stats.cpu().numpy().reshape(B * H, 2),
-                     mask.cpu().numpy().reshape(B * H, T, T) if debug else None,
-                     margin.cpu().numpy().reshape(B * H, T, T) if debug else None)
+                     mask.cpu().numpy().reshape(B * H, T, Tc) if debug else None,
+                     margin.cpu().numpy().reshape(B * H, T, Tc) if debug else None)
 
 
 @dataclass
@@ -80,24 +81,25 @@ class ParityReport:
 
 def compare_head(gpu: GpuResult, bh: int, q_bits, k_bits, v_bits, *, tile: int, mode: int, lam: float,
                  qtiles: Optional[Sequence[int]] = None, report: Optional[ParityReport] = None,
-                 scale: Optional[float] = None) -> ParityReport:
+                 scale: Optional[float] = None, tile_k: Optional[int] = None) -> ParityReport:
     """Compare one head of a GPU run with the oracle on the given decision tiles (all if None)."""
     rep = report if report is not None else ParityReport()
     N, D = q_bits.shape
     T = -(-N // tile)
     qt = list(range(T)) if qtiles is None else list(qtiles)
-    free = oracle.run_head(q_bits, k_bits, v_bits, tile=tile, lam=lam, mode=mode, qtiles=qt, scale=scale)
+    free = oracle.run_head(q_bits, k_bits, v_bits, tile=tile, lam=lam, mode=mode, qtiles=qt, scale=scale, tile_k=tile_k)
     gskip = gpu.skip[bh][qt]                                   # [n, T]
     diverged = [t for t in range(len(qt)) if not np.array_equal(gskip[t], free.skip[t])]
     replay = None
     if diverged:
         replay = oracle.run_head(q_bits, k_bits, v_bits, tile=tile, lam=lam, mode=mode,
-                                 qtiles=[qt[t] for t in diverged], forced_skip=gskip[diverged], scale=scale)
+                                 qtiles=[qt[t] for t in diverged], forced_skip=gskip[diverged], scale=scale,
+                                 tile_k=tile_k)
     for t, i in enumerate(qt):
         rows = min(tile, N - i * tile)
         r0 = i * tile
         rep.tiles_checked += 1
-        rep.decisions_checked += T
+        rep.decisions_checked += gskip.shape[1]
         if t in diverged:
             d = diverged.index(t)
             rep.diverged_qtiles += 1
@@ -148,12 +150,12 @@ def compare_head(gpu: GpuResult, bh: int, q_bits, k_bits, v_bits, *, tile: int, 
     return rep
 
 
-def check_stats(gpu: GpuResult, N: int, tile: int) -> None:
+def check_stats(gpu: GpuResult, N: int, tile: int, tile_k: Optional[int] = None) -> None:
     """stats_out = {executed, skipped} per head must equal the bitmap's counts; executed + skipped = T_r T_c."""
     T = -(-N // tile)
     for bh in range(gpu.stats.shape[0]):
         skipped = int(gpu.skip[bh].sum())
         assert gpu.skip[bh].max() <= 1
         assert gpu.stats[bh, 1] == skipped, (bh, gpu.stats[bh], skipped)
-        assert gpu.stats[bh, 0] + gpu.stats[bh, 1] == T * T
+        assert gpu.stats[bh, 0] + gpu.stats[bh, 1] == T * -(-N // (tile_k or tile))
         assert not gpu.skip[bh][:, 0].any()          # tile 0 never skipped

@@ -1,0 +1,96 @@
+"""GPU parity for decision tiles narrower than the MMA tile (block size 32):
+128 x 64 and 128 x 32 decision tiles at D = 128, against the oracle run with tile_q = 128, tile_k = 64 / 32."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import MODE_DYNAMIC, MODE_FIXED
+from workloads import CONFIGS, f32_to_bf16_bits, make_qkv
+from dataclasses import replace
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def parity():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    import parity_utils
+    return parity_utils
+
+
+def _small_cfg(aligned, grid=(4, 16, 16)):
+    # config 0's grid and generator with D = 128 (the narrow decision tiles exist for D = 128 only)
+    return replace(CONFIGS["cfg0"], name="cfg0_d128", D=128, tile=128, grid=grid, aligned=aligned)
+
+
+@pytest.mark.parametrize("tile_k", [32, 64])
+@pytest.mark.parametrize("aligned", [False, True])
+def test_subtile_decisions_match_oracle(parity, seed, tile_k, aligned):
+    cfg = _small_cfg(aligned)
+    qb, kb, vb = make_qkv(cfg, seed)
+    for mode in (MODE_FIXED, MODE_DYNAMIC):
+        for lam in (-1.0, -2.0, -3.0, -4.0, -6.0):
+            gpu = parity.run_gpu(qb, kb, vb, mode=mode, lam=lam, tile=128, tile_k=tile_k)
+            parity.check_stats(gpu, cfg.N, 128, tile_k)
+            rep = parity.ParityReport()
+            for h in range(cfg.H):
+                parity.compare_head(gpu, h, qb[0, h], kb[0, h], vb[0, h], tile=128, tile_k=tile_k, mode=mode, lam=lam,
+                                    report=rep)
+            print(f"[subtile] tile_k={tile_k} aligned={aligned} mode={mode} lam={lam}: sparsity "
+                  f"{gpu.stats[:, 1].sum() / gpu.stats.sum():.3f} disagree={rep.disagreements} max-abs={rep.max_abs:.2e}")
+            assert rep.ok(), "\n".join(rep.failures[:10])
+
+
+@pytest.mark.parametrize("N,tile_k", [(1000, 32), (2125, 32), (193, 64), (129, 32), (97, 32), (33, 64), (4000, 64)])
+def test_subtile_ragged_random_inputs(parity, seed, N, tile_k):
+    rng = np.random.default_rng([seed, N, tile_k])
+    B, H, D = 1, 2, 128
+    q = rng.standard_normal((B, H, N, D), dtype=np.float32) * 1.3
+    k = rng.standard_normal((B, H, N, D), dtype=np.float32) * 1.3
+    k[:, :, : N // 3] *= 1.6                               # a heavier head of the sequence so that later tiles get skipped
+    v = rng.standard_normal((B, H, N, D), dtype=np.float32)
+    qb, kb, vb = (f32_to_bf16_bits(x) for x in (q, k, v))
+    for mode, lam in ((MODE_DYNAMIC, -3.0), (MODE_DYNAMIC, -6.0), (MODE_FIXED, -2.0)):
+        gpu = parity.run_gpu(qb, kb, vb, mode=mode, lam=lam, tile=128, tile_k=tile_k)
+        parity.check_stats(gpu, N, 128, tile_k)
+        rep = parity.ParityReport()
+        for h in range(H):
+            parity.compare_head(gpu, h, qb[0, h], kb[0, h], vb[0, h], tile=128, tile_k=tile_k, mode=mode, lam=lam, report=rep)
+        assert rep.ok(), "\n".join(rep.failures[:10])
+
+
+def test_subtile_at_bench_shape_sampled(parity, seed):
+    """Config 1's shape (one head) in the launch configuration of the timed runs (no debug outputs for the stats run),
+    oracle on sampled Q tiles: first, ragged last, two random."""
+    cfg = CONFIGS["cfg1_aligned"]
+    qb, kb, vb = make_qkv(cfg, seed, heads=[3])
+    lam = math.log(1.5) + math.log(32 / cfg.N)              # Eq. 7 with B_c = 32
+    plain = parity.run_gpu(qb, kb, vb, mode=MODE_DYNAMIC, lam=lam, tile=128, tile_k=32, debug=False)
+    gpu = parity.run_gpu(qb, kb, vb, mode=MODE_DYNAMIC, lam=lam, tile=128, tile_k=32)
+    assert np.array_equal(plain.stats, gpu.stats) and np.array_equal(plain.out, gpu.out)
+    parity.check_stats(gpu, cfg.N, 128, 32)
+    rep = parity.ParityReport()
+    parity.compare_head(gpu, 0, qb[0, 0], kb[0, 0], vb[0, 0], tile=128, tile_k=32, mode=MODE_DYNAMIC, lam=lam,
+                        qtiles=[0, 255, 77, 190], report=rep)
+    print(f"[subtile] cfg1_aligned head 3: sparsity {gpu.stats[:, 1].sum() / gpu.stats.sum():.3f}")
+    assert rep.ok(), "\n".join(rep.failures[:10])
+
+
+def test_subtile_rejected_where_unsupported():
+    import torch
+    import paper_2606_16317_b200 as sa
+    q = torch.zeros((1, 1, 256, 64), device="cuda", dtype=torch.bfloat16)
+    out = torch.empty_like(q)
+    with pytest.raises(sa.SparseAttnError) as e:           # D = 64 has 64 x 64 decision tiles only
+        sa.sparse_attn_fwd(q, q, q, out, None, 1, 1, 256, 64, sa.make_params(lam=-3.0, tile_q=64, tile_k=32),
+                           sa.MODE_DYNAMIC, None)
+    assert e.value.status == -4
+    q = torch.zeros((1, 1, 256, 128), device="cuda", dtype=torch.bfloat16)
+    out = torch.empty_like(q)
+    with pytest.raises(sa.SparseAttnError) as e:           # DENSE mode takes no decisions
+        sa.sparse_attn_fwd(q, q, q, out, None, 1, 1, 256, 128, sa.make_params(tile_q=128, tile_k=32), sa.MODE_DENSE, None)
+    assert e.value.status == -4
