@@ -55,8 +55,7 @@ def executed_flop(BH, N, D, tile, stats):
     """QK^T for every tile + P V for executed tiles; ragged tiles counted as full
     in the P V term (error < 1/T_c)."""
     qk = 2.0 * BH * N * N * D
-    T = -(-N // tile)
-    frac_exec = float(stats[..., 0].sum()) / float(BH * T * T)
+    frac_exec = float(stats[..., 0].sum()) / float(stats.sum())   # executed / all decision tiles (any tile_k)
     return qk + 2.0 * BH * N * N * D * frac_exec
 
 
@@ -158,11 +157,11 @@ def workload_name(cfg):
 
 
 # ---------------------------------------------------------------------------------------------- GPU arm
-def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier, sampler=None):
+def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier, sampler=None, tile_k=0):
     """Returns (total_ms over `steps` calls, per-call ms list, stats [B,H,2])."""
     q, k, v, out, lse, stats = bufs
     stream = torch.cuda.current_stream()
-    p = sa.make_params(lam=lam, stream=stream.cuda_stream)
+    p = sa.make_params(lam=lam, stream=stream.cuda_stream, tile_q=cfg.tile if tile_k else 0, tile_k=tile_k)
     for _ in range(warmup):
         sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p, mode, stats)
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
@@ -300,18 +299,20 @@ def main():
         stats = torch.zeros((cfg.B, cfg.H, 2), device="cuda", dtype=torch.int64)
         bufs = (q, k, v, out, lse, stats)
         res = {}
-        for mname, mode, mlam in (("dense", sa.MODE_DENSE, -math.inf), ("fixed", sa.MODE_FIXED, lam),
-                                  ("dynamic", sa.MODE_DYNAMIC, lam)):
-            if mname not in args.modes.split(","):
+        lam32 = math.log(P_REAL) + math.log(32 / cfg.N)       # Eq. 7 with B_c = 32
+        for mname, mode, mlam, mtk in (("dense", sa.MODE_DENSE, -math.inf, 0), ("fixed", sa.MODE_FIXED, lam, 0),
+                                       ("dynamic", sa.MODE_DYNAMIC, lam, 0),
+                                       ("dynamic_bc32", sa.MODE_DYNAMIC, lam32, 32)):
+            if mname.split("_")[0] not in args.modes.split(",") or (mtk and (args.no_aligned or cfg.D != 128)):
                 continue
             headline = (vi == 0 and mname == "dynamic")
             if headline:
                 l0 = sa.launch_count()
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler)
+                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk)
                 headline_launches = sa.launch_count() - l0 - args.warmup
                 head_total_ms = total
             else:
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler)
+                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk)
             if dist is not None:
                 t = torch.tensor([total], device="cuda")
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -342,13 +343,16 @@ def main():
                 "executed_flop_per_launch_rank0": executed_flop(BH, cfg.N, cfg.D, cfg.tile, st[None]),
                 **quality,
             }
-        for mname in ("fixed", "dynamic"):
+        for mname in ("fixed", "dynamic", "dynamic_bc32"):
             if mname not in res or "dense" not in res:
                 continue
+            if mname == "dynamic_bc32":
+                res[mname]["lambda"] = lam32
+                res[mname]["decision_tile"] = "128x32"
             res[mname]["speedup_vs_dense"] = res["dense"]["ms"] / res[mname]["ms"]
             res[mname]["mma_bound_model"] = 1.0 / (1.0 - res[mname]["sparsity"] / 2.0)
         if brick is not None and reorder_info is not None:
-            for mname in ("fixed", "dynamic"):
+            for mname in ("fixed", "dynamic", "dynamic_bc32"):
                 if mname in res and "dense" in results.get(variants[0][0], {}):
                     # whole re-ordered pipeline (3 gathers + attention + 1 scatter) against the plain DENSE call
                     res[mname]["ms_with_reorder"] = res[mname]["ms"] + reorder_info["ms_4_passes"]

@@ -140,7 +140,8 @@ struct SmemLayout {
     static constexpr int kLockOff = kVotesOff + 256;
     static constexpr int kProgOff = kLockOff + 32;
     static constexpr int kPvMaskOff = kProgOff + 16;       // pvmask[2][4]: kept sub-tiles of tile j (SUB > 1), ring like votes
-    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16 + 32;
+    static constexpr int kPreOff = kPvMaskOff + 32;        // pre[2][2][4]: preliminary sub-tile votes per warp (SUB > 1)
+    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16 + 32 + 64;
     static constexpr int kTotal = kMiscOff + kMiscBytes;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
     static_assert(kDynamicBytes <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
@@ -423,9 +424,11 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         mbar_wait(p_ready(x), ppar[x]);
                         tc_fence_after();
                         ppar[x] ^= 1u;
+                        uint32_t pvmask2 = 0xffu;            // the mask is complete once all of P_x has been handed over
+                        if (SUB > 1) pvmask2 = ld_shared_u32(sbase + L::kPvMaskOff + (x * 4 + (j & 3)) * 4);
                         TRACE(2)
                         if (elect_one_sync()) {
-                            issue_pv(x, vaddr, true, 1, pvmask);
+                            issue_pv(x, vaddr, true, 1, pvmask2);
                             umma_commit(v_empty(vslot));     // this slot's P_x V_j has read V_j
                             if (has_next) {
                                 issue_qk(x, kaddr, kEarlyB ? 0 : 2);   // (again, if a speculative one was overwritten by P_x)
@@ -566,19 +569,54 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const float neg_m = -m_used;
                 const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
                 const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
+                // Row maxima of the SUB decision tiles (a3), then a PRELIMINARY test of all of them against the
+                // statistics as they stand before this MMA tile.  Within the tile the reference (LSE, or the running
+                // max) can only grow, so t can only shrink: a sub-tile skipped by the preliminary test is skipped by
+                // the sequential rule too.  One vote round settles every skipped sub-tile (all of them in a run of
+                // skipped tiles); only sub-tiles that pass it AND follow a retained one are tested again.
+                float msub[SUB];
+#pragma unroll
+                for (int s = 0; s < SUB; ++s) {
+                    float ma = S_AT(s * W), mb = S_AT(s * W + 1), mc = S_AT(s * W + 2), md = S_AT(s * W + 3);
+#pragma unroll
+                    for (int c = 4; c + 8 <= W; c += 8) {    // 4 independent 3-input max chains
+                        ma = fmax3(ma, S_AT(s * W + c), S_AT(s * W + c + 1));
+                        mb = fmax3(mb, S_AT(s * W + c + 2), S_AT(s * W + c + 3));
+                        mc = fmax3(mc, S_AT(s * W + c + 4), S_AT(s * W + c + 5));
+                        md = fmax3(md, S_AT(s * W + c + 6), S_AT(s * W + c + 7));
+                    }
+                    ma = fmax3(ma, S_AT(s * W + W - 4), S_AT(s * W + W - 3));
+                    mb = fmax3(mb, S_AT(s * W + W - 2), S_AT(s * W + W - 1));
+                    msub[s] = fmaxf(fmaxf(ma, mb), fmaxf(mc, md)) * scale_log2;
+                }
+                uint32_t cand = (1u << SUB) - 1u;            // bit s: sub-tile s passed the preliminary test
+                if (!kDebug) {                               // (debug builds test every sub-tile in sequence: margins)
+                    const float ref0 = (mode == kModeDynamic) ? lse2 : m_true;
+                    uint32_t wc = 0u;
+#pragma unroll
+                    for (int s = 0; s < SUB; ++s) {
+                        const bool rs = (j * SUB + s > 0) && (!row_valid || (msub[s] - ref0 < lambda_log2));
+                        if (!__all_sync(0xffffffffu, rs)) wc |= 1u << s;
+                    }
+                    volatile uint32_t* pre = reinterpret_cast<volatile uint32_t*>(smem + L::kPreOff) + (x * 2 + (j & 1)) * 4;
+                    if (lane == 0) pre[w] = wc;
+                    named_bar_sync(1 + x, 128);
+                    cand = pre[0] | pre[1] | pre[2] | pre[3];
+                }
                 uint32_t kept = 0u;                          // bit s: decision sub-tile s retained
+                bool half_sent = false;
 #pragma unroll
                 for (int s = 0; s < SUB; ++s) {
                     const int jj = j * SUB + s;              // decision tile index along the keys
                     if (jj >= a.T_c_dec) break;              // beyond the last key (ragged tail): no such tile
-                    float ms = S_AT(s * W);
-#pragma unroll
-                    for (int c = 1; c < W; ++c) ms = fmaxf(ms, S_AT(s * W + c));
-                    ms *= scale_log2;                        // a3 for this decision tile
+                    const float ms = msub[s];
                     const float ref = (mode == kModeDynamic) ? lse2 : m_true;
                     const float t2 = ms - ref;               // Eq. 5, log2 units (+inf before the first retained tile)
                     const bool row_skip = (jj > 0) && (!row_valid || (t2 < lambda_log2));
-                    const bool skip_s = named_bar_red_and(1 + x, 128, row_skip);   // all 128 rows of the Q tile (R1)
+                    bool skip_s;
+                    if (!((cand >> s) & 1u)) skip_s = true;  // settled by the preliminary round
+                    else if (!kDebug && kept == 0u) skip_s = false;   // statistics unchanged since that round
+                    else skip_s = named_bar_red_and(1 + x, 128, row_skip);   // all 128 rows of the Q tile (R1)
                     if (kDebug) {
                         float gm = INFINITY;
                         if (want_margin) {
@@ -638,6 +676,15 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     unpack_f32x2(rs2, r0, r1);
                     l += r0 + r1;                            // the next decision of this tile needs the new LSE (Eq. 6)
                     if (mode == kModeDynamic) lse2 = m_used + fast_log2(l);
+                    if (s == SUB / 2 - 1) {
+                        // the first half of the keys is done and something in it was retained: hand it over now, so
+                        // that its P V steps run while the second half is decided and exponentiated
+                        if (w == 0 && lane == 0) st_shared_u32(sbase + L::kPvMaskOff + (x * 4 + q) * 4, kept);
+                        tmem_wait_st();
+                        tc_fence_before();
+                        mbar_arrive(p_half(x));
+                        half_sent = true;
+                    }
                 }
                 prev_skip = kept == 0u;
                 if (kept == 0u) {                            // every sub-tile skipped: the MMA tile is skipped
@@ -652,7 +699,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 if (w == 0 && lane == 0) st_shared_u32(sbase + L::kPvMaskOff + (x * 4 + q) * 4, kept);
                 tmem_wait_st();
                 tc_fence_before();
-                mbar_arrive(p_half(x));                      // (release: the mask above is visible to the issuer)
+                if (!half_sent) mbar_arrive(p_half(x));      // (release: the mask above is visible to the issuer)
                 mbar_arrive(p_ready(x));
                 continue;
             }
