@@ -140,8 +140,9 @@ struct SmemLayout {
     static constexpr int kLockOff = kVotesOff + 256;
     static constexpr int kProgOff = kLockOff + 32;
     static constexpr int kPvMaskOff = kProgOff + 16;       // pvmask[2][4]: kept sub-tiles of tile j (SUB > 1), ring like votes
-    static constexpr int kPreOff = kPvMaskOff + 32;        // pre[2][2][4]: preliminary sub-tile votes per warp (SUB > 1)
-    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16 + 32 + 64;
+    static constexpr int kPreOff = kPvMaskOff + 32;        // pre[2][4][4]: per-warp votes on sub-tiles (SUB > 1): buffers 0, 1
+                                                           // preliminary round of tile j (by parity), 2, 3 later rounds
+    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16 + 32 + 128;
     static constexpr int kTotal = kMiscOff + kMiscBytes;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
     static_assert(kDynamicBytes <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
@@ -589,34 +590,92 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     mb = fmax3(mb, S_AT(s * W + W - 2), S_AT(s * W + W - 1));
                     msub[s] = fmaxf(fmaxf(ma, mb), fmaxf(mc, md)) * scale_log2;
                 }
-                uint32_t cand = (1u << SUB) - 1u;            // bit s: sub-tile s passed the preliminary test
+                uint32_t cand = (1u << SUB) - 1u;            // bit s: sub-tile s passed the preliminary test; bit SUB+s: kept for certain
                 if (!kDebug) {                               // (debug builds test every sub-tile in sequence: margins)
                     const float ref0 = (mode == kModeDynamic) ? lse2 : m_true;
+                    // Upper bound of how far the reference of this row can grow inside the tile, whatever is retained:
+                    // LSE' <= log2(2^LSE + BC * 2^mhat) (DYNAMIC), m' <= max(m, mhat) (FIXED).  A row whose t stays
+                    // >= lambda even against that bound keeps its sub-tile for certain, with no second vote (bits
+                    // SUB..2 SUB-1).  1e-3 covers the rounding of the approximate ex2 / lg2 in the running statistics.
+                    const float grow = ((mode == kModeDynamic) ? fast_log2(1.f + static_cast<float>(BC) * fast_exp2(mhat2 - ref0))
+                                                               : fmaxf(0.f, mhat2 - ref0)) + 1e-3f;
                     uint32_t wc = 0u;
 #pragma unroll
                     for (int s = 0; s < SUB; ++s) {
                         const bool rs = (j * SUB + s > 0) && (!row_valid || (msub[s] - ref0 < lambda_log2));
                         if (!__all_sync(0xffffffffu, rs)) wc |= 1u << s;
+                        const bool sure = row_valid && (msub[s] - ref0 - grow >= lambda_log2);
+                        if (__any_sync(0xffffffffu, sure)) wc |= 1u << (SUB + s);
                     }
-                    volatile uint32_t* pre = reinterpret_cast<volatile uint32_t*>(smem + L::kPreOff) + (x * 2 + (j & 1)) * 4;
+                    volatile uint32_t* pre = reinterpret_cast<volatile uint32_t*>(smem + L::kPreOff) + (x * 4 + (j & 1)) * 4;
                     if (lane == 0) pre[w] = wc;
                     named_bar_sync(1 + x, 128);
                     cand = pre[0] | pre[1] | pre[2] | pre[3];
                 }
                 uint32_t kept = 0u;                          // bit s: decision sub-tile s retained
                 bool half_sent = false;
+                // Row sums of retained sub-tiles are folded into l (and LSE) lazily: only a decision that is still open
+                // needs the new LSE (Eq. 6); between sub-tiles that are settled the ex2 streams run back to back.
+                uint64_t acc2 = pack_f32x2(0.f, 0.f);
+                bool dirty = false;
+                auto fold = [&]() {
+                    if (dirty) {
+                        float r0, r1;
+                        unpack_f32x2(acc2, r0, r1);
+                        l += r0 + r1;
+                        if (mode == kModeDynamic) lse2 = m_used + fast_log2(l);
+                        acc2 = pack_f32x2(0.f, 0.f);
+                        dirty = false;
+                    }
+                };
 #pragma unroll
                 for (int s = 0; s < SUB; ++s) {
                     const int jj = j * SUB + s;              // decision tile index along the keys
                     if (jj >= a.T_c_dec) break;              // beyond the last key (ragged tail): no such tile
                     const float ms = msub[s];
+                    const bool open = ((cand >> s) & 1u) && (kDebug || (kept != 0u && !((cand >> (SUB + s)) & 1u)));
+                    if (open) fold();                        // this decision is taken with the current statistics
                     const float ref = (mode == kModeDynamic) ? lse2 : m_true;
                     const float t2 = ms - ref;               // Eq. 5, log2 units (+inf before the first retained tile)
                     const bool row_skip = (jj > 0) && (!row_valid || (t2 < lambda_log2));
-                    bool skip_s;
-                    if (!((cand >> s) & 1u)) skip_s = true;  // settled by the preliminary round
-                    else if (!kDebug && kept == 0u) skip_s = false;   // statistics unchanged since that round
-                    else skip_s = named_bar_red_and(1 + x, 128, row_skip);   // all 128 rows of the Q tile (R1)
+                    uint64_t rs2 = pack_f32x2(0.f, 0.f);     // row sum of this sub-tile, two packed chains
+                    auto exp_sub = [&]() {                   // a5 for this sub-tile: P columns and row sum
+#pragma unroll
+                        for (int c = s * (W / 32); c < (s + 1) * (W / 32); ++c) {
+                            uint32_t pk[16];
+#pragma unroll
+                            for (int i = 0; i < 16; ++i) {
+                                float x0, x1;
+                                unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(su[c][2 * i]), __uint_as_float(su[c][2 * i + 1])),
+                                                       scale2, negm2), x0, x1);
+                                const float p0 = fast_exp2(x0);
+                                const float p1 = fast_exp2(x1);
+                                rs2 = add_f32x2(rs2, pack_f32x2(p0, p1));
+                                pk[i] = pack_bf16x2(p0, p1);
+                            }
+                            tmem_st_x16(tS + c * 16, pk);
+                        }
+                    };
+                    bool skip_s, did_exp = false;
+                    if (!((cand >> s) & 1u)) {
+                        skip_s = true;                       // settled by the preliminary round
+                    } else if (!kDebug && (kept == 0u || ((cand >> (SUB + s)) & 1u))) {
+                        skip_s = false;                      // statistics unchanged since that round, or kept for certain
+                    } else if (kept != 0u) {
+                        // A sub-tile that follows a retained one is exponentiated BEFORE its vote is settled: the
+                        // all-rows vote (shared-memory words + one barrier) then completes in the shadow of the ex2
+                        // work instead of holding it up.  If the vote says skip, the P columns just written are never
+                        // read (mask bit clear) and the row sum is dropped.
+                        exp_sub();
+                        did_exp = true;
+                        const bool wv = __all_sync(0xffffffffu, row_skip);
+                        volatile uint32_t* sv = reinterpret_cast<volatile uint32_t*>(smem + L::kPreOff) + (x * 4 + 2 + (s & 1)) * 4;
+                        if (lane == 0) sv[w] = wv ? 1u : 0u;
+                        named_bar_sync(1 + x, 128);
+                        skip_s = (sv[0] & sv[1] & sv[2] & sv[3]) != 0u;   // all 128 rows of the Q tile (R1)
+                    } else {
+                        skip_s = named_bar_red_and(1 + x, 128, row_skip);
+                    }
                     if (kDebug) {
                         float gm = INFINITY;
                         if (want_margin) {
@@ -656,26 +715,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     }
                     kept |= 1u << s;
                     m_true = fmaxf(m_true, ms);
-                    uint64_t rs2 = pack_f32x2(0.f, 0.f);
-#pragma unroll
-                    for (int c = s * (W / 32); c < (s + 1) * (W / 32); ++c) {
-                        uint32_t pk[16];
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) {
-                            float x0, x1;
-                            unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(su[c][2 * i]), __uint_as_float(su[c][2 * i + 1])),
-                                                   scale2, negm2), x0, x1);
-                            const float p0 = fast_exp2(x0);
-                            const float p1 = fast_exp2(x1);
-                            rs2 = add_f32x2(rs2, pack_f32x2(p0, p1));
-                            pk[i] = pack_bf16x2(p0, p1);
-                        }
-                        tmem_st_x16(tS + c * 16, pk);
-                    }
-                    float r0, r1;
-                    unpack_f32x2(rs2, r0, r1);
-                    l += r0 + r1;                            // the next decision of this tile needs the new LSE (Eq. 6)
-                    if (mode == kModeDynamic) lse2 = m_used + fast_log2(l);
+                    if (!did_exp) exp_sub();
+                    acc2 = add_f32x2(acc2, rs2);
+                    dirty = true;
                     if (s == SUB / 2 - 1) {
                         // the first half of the keys is done and something in it was retained: hand it over now, so
                         // that its P V steps run while the second half is decided and exponentiated
@@ -701,6 +743,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 tc_fence_before();
                 if (!half_sent) mbar_arrive(p_half(x));      // (release: the mask above is visible to the issuer)
                 mbar_arrive(p_ready(x));
+                fold();                                      // statistics for the next tile, behind the hand-over
                 continue;
             }
             // ---- predicate and all-rows vote (a4)

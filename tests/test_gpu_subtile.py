@@ -40,6 +40,15 @@ def test_subtile_decisions_match_oracle(parity, seed, tile_k, aligned):
             for h in range(cfg.H):
                 parity.compare_head(gpu, h, qb[0, h], kb[0, h], vb[0, h], tile=128, tile_k=tile_k, mode=mode, lam=lam,
                                     report=rep)
+            # the timed (non-debug) build settles sub-tiles by a preliminary round, a certain-keep bound and lazy
+            # statistics: its counts must equal the oracle's and its output must be within the same tolerance
+            plain = parity.run_gpu(qb, kb, vb, mode=mode, lam=lam, tile=128, tile_k=tile_k, debug=False)
+            for h in range(cfg.H):
+                ref = oracle.run_head(qb[0, h], kb[0, h], vb[0, h], tile=128, tile_k=tile_k, lam=lam, mode=mode)
+                assert (int(plain.stats[h, 0]), int(plain.stats[h, 1])) == (ref.executed, ref.skipped)
+                err = np.abs(plain.out[h] - ref.rows()[0])
+                assert err.max() < parity.OUT_MAX_ABS and err.mean() < parity.OUT_MEAN_ABS
+                assert np.abs(plain.lse[h] - ref.rows()[1]).max() < parity.LSE_ABS
             print(f"[subtile] tile_k={tile_k} aligned={aligned} mode={mode} lam={lam}: sparsity "
                   f"{gpu.stats[:, 1].sum() / gpu.stats.sum():.3f} disagree={rep.disagreements} max-abs={rep.max_abs:.2e}")
             assert rep.ok(), "\n".join(rep.failures[:10])
@@ -71,7 +80,11 @@ def test_subtile_at_bench_shape_sampled(parity, seed):
     lam = math.log(1.5) + math.log(32 / cfg.N)              # Eq. 7 with B_c = 32
     plain = parity.run_gpu(qb, kb, vb, mode=MODE_DYNAMIC, lam=lam, tile=128, tile_k=32, debug=False)
     gpu = parity.run_gpu(qb, kb, vb, mode=MODE_DYNAMIC, lam=lam, tile=128, tile_k=32)
-    assert np.array_equal(plain.stats, gpu.stats) and np.array_equal(plain.out, gpu.out)
+    # the debug build folds the row sums after every sub-tile, the plain build lazily: same decisions, and outputs
+    # equal up to the rounding order of l (at most one bf16 ulp of the output here and there)
+    assert np.array_equal(plain.stats, gpu.stats)
+    d = np.abs(plain.out - gpu.out)
+    assert d.max() <= 2e-2 and d.mean() < 1e-4
     parity.check_stats(gpu, cfg.N, 128, 32)
     rep = parity.ParityReport()
     parity.compare_head(gpu, 0, qb[0, 0], kb[0, 0], vb[0, 0], tile=128, tile_k=32, mode=MODE_DYNAMIC, lam=lam,
