@@ -26,8 +26,13 @@ enum sparse_attn_mode {
     SPARSE_ATTN_DENSE = 0,   /* no skipping: softmax(scale * Q K^T) V, FlashAttention-2 tiling */
     SPARSE_ATTN_FIXED = 1,   /* BLASST-style: skip tile j iff  mhat_r - m_r^(j-1) < lambda  for every valid row r
                                 (tile max minus running max over retained tiles) */
-    SPARSE_ATTN_DYNAMIC = 2  /* DynSparse: skip tile j iff  t_r = mhat_r - LSE_r^(j-1) < lambda  for every valid row r,
+    SPARSE_ATTN_DYNAMIC = 2, /* DynSparse: skip tile j iff  t_r = mhat_r - LSE_r^(j-1) < lambda  for every valid row r,
                                 LSE over the retained tiles only (Eq. 5-6) */
+    SPARSE_ATTN_MASK = 3     /* mask-driven: the decisions are READ from params->skip_mask_in instead of being taken in the
+                                loop -- the block-mask methods the paper compares with (Top-K, Top-P, the "ideal" mask of
+                                section 3; Fig. 3) run through the same kernel.  Everything else
+                                is as in the other sparse modes: retained tiles only enter m, l, O and lse (Eq. 1, Eq. 6).
+                                Tile j = 0 of every row of tiles is retained whatever its byte says. */
 };
 
 /* return codes: 0 on success, negative on error */
@@ -37,9 +42,10 @@ enum sparse_attn_status {
     SPARSE_ATTN_ERR_SHAPE = -2,        /* B, H or N <= 0, or B*H / N too large for the launch */
     SPARSE_ATTN_ERR_HEAD_DIM = -3,     /* D not in {64, 128} */
     SPARSE_ATTN_ERR_TILE = -4,         /* tile_q / tile_k not a supported decision tile for this D and mode */
-    SPARSE_ATTN_ERR_MODE = -5,         /* mode not in {0, 1, 2} */
+    SPARSE_ATTN_ERR_MODE = -5,         /* mode not in {0, 1, 2, 3} */
     SPARSE_ATTN_ERR_PARAMS = -6,       /* params NULL in a sparse mode, struct_size wrong, lambda NaN,
-                                          lambda > 0 in FIXED mode, softmax_scale negative / non-finite */
+                                          lambda > 0 in FIXED mode, softmax_scale negative / non-finite,
+                                          skip_mask_in NULL in MASK mode or set in another mode */
     SPARSE_ATTN_ERR_ALIGNMENT = -7,    /* q, k, v or out not 16-byte aligned (TMA / vector stores) */
     SPARSE_ATTN_ERR_DEVICE = -8,       /* no CUDA device, or the current device is not sm_100 (B200) */
     SPARSE_ATTN_ERR_CUDA = -9          /* a CUDA runtime / driver call failed; see sparse_attn_last_error() */
@@ -64,7 +70,10 @@ typedef struct sparse_attn_params {
     uint8_t* skip_mask_out; /* optional, device, [B, H, T_r, T_c] bytes, 1 = tile skipped, fully overwritten.
                                T_r = ceil(N / tile_q), T_c = ceil(N / tile_k).  NULL in timed runs. */
     float* margin_out;      /* optional, device, [B, H, T_r, T_c] fp32: g_ij = max_r t_r - lambda as evaluated on
-                               the GPU (+inf for tile 0 and in DENSE mode).  Debug / parity only. */
+                               the GPU (+inf for tile 0 and in DENSE mode; in MASK mode the DYNAMIC margin of the state
+                               the mask built).  Debug / parity only. */
+    const uint8_t* skip_mask_in; /* MASK mode only (must be NULL otherwise): device, [B, H, T_r, T_c] bytes, non-zero =
+                               skip the tile; never written.  Default decision tiles only (tile_q = tile_k = default). */
 } sparse_attn_params;
 
 /*

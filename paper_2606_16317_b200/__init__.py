@@ -8,6 +8,7 @@ from .binding import (  # noqa: F401
     MODE_DENSE,
     MODE_DYNAMIC,
     MODE_FIXED,
+    MODE_MASK,
     SparseAttnError,
     SparseAttnParams,
     lambda_from_preal,

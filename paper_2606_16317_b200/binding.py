@@ -11,7 +11,7 @@ import ctypes
 import os
 from typing import Optional
 
-MODE_DENSE, MODE_FIXED, MODE_DYNAMIC = 0, 1, 2
+MODE_DENSE, MODE_FIXED, MODE_DYNAMIC, MODE_MASK = 0, 1, 2, 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("SPARSE_ATTN_LIB") or os.path.join(_HERE, "libsparse_attn.so")
@@ -50,6 +50,7 @@ class SparseAttnParams(ctypes.Structure):
         ("stream", ctypes.c_void_p),
         ("skip_mask_out", ctypes.c_void_p),
         ("margin_out", ctypes.c_void_p),
+        ("skip_mask_in", ctypes.c_void_p),
     ]
 
 
@@ -128,7 +129,7 @@ def _ptr(x) -> Optional[int]:
 
 
 def make_params(lam: float = float("-inf"), softmax_scale: float = 0.0, tile_q: int = 0, tile_k: int = 0,
-                stream=None, skip_mask_out=None, margin_out=None) -> SparseAttnParams:
+                stream=None, skip_mask_out=None, margin_out=None, skip_mask_in=None) -> SparseAttnParams:
     p = SparseAttnParams()
     p.struct_size = ctypes.sizeof(SparseAttnParams)
     p.lambda_ = lam
@@ -138,6 +139,7 @@ def make_params(lam: float = float("-inf"), softmax_scale: float = 0.0, tile_q: 
     p.stream = _ptr(stream)
     p.skip_mask_out = _ptr(skip_mask_out)
     p.margin_out = _ptr(margin_out)
+    p.skip_mask_in = _ptr(skip_mask_in)
     return p
 
 

@@ -53,7 +53,7 @@ namespace dsa {
 #define PROF_FLUSH(base, n, cond)
 #endif
 
-enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2 };
+enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2, kModeMask = 3 };
 
 constexpr int kNumThreads = 384;      // 3 warpgroups
 constexpr int kKProducerWarp = 8;
@@ -108,6 +108,7 @@ struct FwdArgs {
     unsigned long long* stats;   // [BH, 2] or null (pre-zeroed)
     uint8_t* skip_mask;          // [BH, T_r, T_c_dec] or null
     float* margin;               // [BH, T_r, T_c_dec] or null
+    const uint8_t* mask_in;      // MASK mode: [BH, T_r, T_c] bytes, non-zero = skip (tile 0 is kept regardless)
     int N;
     int T_r;                     // decision tiles along queries
     int T_c;                     // K tiles of BC keys (MMA tiles)
@@ -753,9 +754,11 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 // votes[x][j & 1][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
                 // The MMA warp combines the four votes itself (barrier dec, one arrival per warp), so an all-skip
                 // decision reaches the tensor pipe without the four warps first synchronising with each other.
-                const float ref = (mode == kModeDynamic) ? lse2 : m_true;
+                const float ref = (mode == kModeFixed) ? m_true : lse2;
                 const float t2 = mhat2 - ref;                // Eq. 5 in log2 units (+inf at j = 0: tile 0 is kept)
-                const bool row_skip = (j > 0) && (!row_valid || (t2 < lambda_log2));
+                bool row_skip = (j > 0) && (!row_valid || (t2 < lambda_log2));
+                if (mode == kModeMask)                       // decisions read from the bitmap (one byte per decision tile)
+                    row_skip = (j > 0) && (!grp_valid || __ldg(a.mask_in + tile_row + j) != 0);
                 const bool wskip = __all_sync(0xffffffffu, row_skip);
                 const int q = j & 3;
                 volatile int* vt = votes + (x * 4 + q) * 4;     // ring of 4 tiles (see dec)
@@ -933,7 +936,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             // must not sit between the last exp and the arrive (in-order issue would stall the arrive on them)
             if (!(kSparse && G == 2 && skip_grp)) {
                 l += rs0 + rs1;
-                if (kSparse && mode == kModeDynamic && !(DSA_EXP & 16)) lse2 = m_used + fast_log2(l);
+                if (kSparse && mode != kModeFixed && !(DSA_EXP & 16)) lse2 = m_used + fast_log2(l);
             }
             PROF_TICK(7)
         }

@@ -97,6 +97,7 @@ struct Resolved {
     cudaStream_t stream;
     uint8_t* skip_mask;
     float* margin;
+    const uint8_t* mask_in;
 };
 
 // Host-side validation shared by the device and host-buffer entry points.
@@ -104,7 +105,7 @@ int validate(const void* q, const void* k, const void* v, void* out, int B, int 
              const sparse_attn_params* p, int mode, Resolved* r) {
     g_last_error[0] = '\0';
     if (!q || !k || !v || !out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "q, k, v and out must not be NULL");
-    if (mode < SPARSE_ATTN_DENSE || mode > SPARSE_ATTN_DYNAMIC) return fail(SPARSE_ATTN_ERR_MODE, "mode %d not in {0,1,2}", mode);
+    if (mode < SPARSE_ATTN_DENSE || mode > SPARSE_ATTN_MASK) return fail(SPARSE_ATTN_ERR_MODE, "mode %d not in {0,1,2,3}", mode);
     if (B <= 0 || H <= 0 || N <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N must be positive (got %d, %d, %d)", B, H, N);
     if (static_cast<long long>(B) * H > 65535) return fail(SPARSE_ATTN_ERR_SHAPE, "B*H = %lld exceeds 65535", (long long)B * H);
     if (N > (1 << 24)) return fail(SPARSE_ATTN_ERR_SHAPE, "N = %d exceeds 2^24", N);
@@ -117,6 +118,7 @@ int validate(const void* q, const void* k, const void* v, void* out, int B, int 
     r->stream = nullptr;
     r->skip_mask = nullptr;
     r->margin = nullptr;
+    r->mask_in = nullptr;
     if (p) {
         if (p->struct_size != sizeof(sparse_attn_params))
             return fail(SPARSE_ATTN_ERR_PARAMS, "params->struct_size = %u, expected %zu", p->struct_size, sizeof(sparse_attn_params));
@@ -138,6 +140,14 @@ int validate(const void* q, const void* k, const void* v, void* out, int B, int 
         r->stream = static_cast<cudaStream_t>(p->stream);
         r->skip_mask = p->skip_mask_out;
         r->margin = p->margin_out;
+        if (mode == SPARSE_ATTN_MASK) {
+            if (!p->skip_mask_in) return fail(SPARSE_ATTN_ERR_PARAMS, "MASK mode needs params->skip_mask_in");
+            if (tq != def_tile || tk != def_tile)
+                return fail(SPARSE_ATTN_ERR_TILE, "MASK mode takes the default %dx%d decision tiles only", def_tile, def_tile);
+        } else if (p->skip_mask_in) {
+            return fail(SPARSE_ATTN_ERR_PARAMS, "skip_mask_in is set but mode %d is not MASK", mode);
+        }
+        r->mask_in = p->skip_mask_in;
     }
     return 0;
 }
@@ -185,6 +195,7 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     a.stats = reinterpret_cast<unsigned long long*>(stats_out);
     a.skip_mask = r.skip_mask;
     a.margin = r.margin;
+    a.mask_in = r.mask_in;
     a.N = N;
     a.T_r = (N + r.tile_q - 1) / r.tile_q;
     a.T_c = (N + mma_k - 1) / mma_k;
@@ -233,10 +244,11 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     float *dlse = nullptr, *dmargin = nullptr;
     int64_t* dstats = nullptr;
     uint8_t* dmask = nullptr;
+    uint8_t* dmask_in = nullptr;
     cudaStream_t st = r.stream;
     auto cleanup = [&]() {
         cudaFree(dq); cudaFree(dk); cudaFree(dv); cudaFree(dout); cudaFree(dlse); cudaFree(dstats);
-        cudaFree(dmask); cudaFree(dmargin);
+        cudaFree(dmask); cudaFree(dmargin); cudaFree(dmask_in);
     };
 #define HOST_TRY(expr)                                                                                   \
     do {                                                                                                 \
@@ -254,6 +266,10 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     if (stats_out) HOST_TRY(cudaMalloc(&dstats, BH * 2 * sizeof(int64_t)));
     if (r.skip_mask) HOST_TRY(cudaMalloc(&dmask, BH * T_r * T_c));
     if (r.margin) HOST_TRY(cudaMalloc(&dmargin, BH * T_r * T_c * sizeof(float)));
+    if (r.mask_in) {                                        // MASK mode: the bitmap is a host buffer here too
+        HOST_TRY(cudaMalloc(&dmask_in, BH * T_r * T_c));
+        HOST_TRY(cudaMemcpyAsync(dmask_in, r.mask_in, BH * T_r * T_c, cudaMemcpyHostToDevice, st));
+    }
     HOST_TRY(cudaMemcpyAsync(dq, q, n_elem * 2, cudaMemcpyHostToDevice, st));
     HOST_TRY(cudaMemcpyAsync(dk, k, n_elem * 2, cudaMemcpyHostToDevice, st));
     HOST_TRY(cudaMemcpyAsync(dv, v, n_elem * 2, cudaMemcpyHostToDevice, st));
@@ -264,6 +280,7 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     if (!params) dp.lambda = -INFINITY;
     dp.skip_mask_out = dmask;
     dp.margin_out = dmargin;
+    dp.skip_mask_in = dmask_in;
     rc = sparse_attn_fwd(dq, dk, dv, dout, dlse, B, H, N, D, &dp, mode, dstats);
     if (rc) { cleanup(); return rc; }
     HOST_TRY(cudaMemcpyAsync(out, dout, n_elem * 2, cudaMemcpyDeviceToHost, st));

@@ -38,9 +38,10 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_params_struct_matches_header_layout():
-    # uint32, float, float, int32, int32, (pad), void*, uint8_t*, float*
-    assert ctypes.sizeof(sa.SparseAttnParams) == 48
+    # uint32, float, float, int32, int32, (pad), void*, uint8_t*, float*, const uint8_t*
+    assert ctypes.sizeof(sa.SparseAttnParams) == 56
     assert sa.SparseAttnParams.stream.offset == 24
+    assert sa.SparseAttnParams.skip_mask_in.offset == 48
 
 
 def test_lambda_helpers():
@@ -59,6 +60,7 @@ def _bufs(n=4096):
     ("null_q", -1), ("null_out", -1), ("bad_B", -2), ("bad_N", -2), ("bad_D", -3), ("bad_tile", -4),
     ("bad_mode", -5), ("null_params_sparse", -6), ("nan_lambda", -6), ("positive_lambda_fixed", -6),
     ("bad_struct_size", -6), ("negative_scale", -6), ("misaligned", -7), ("too_many_heads", -2),
+    ("mask_mode_without_mask", -6), ("mask_in_other_mode", -6), ("mask_mode_narrow_tile", -4),
 ])
 def test_error_paths_checked_on_host(case, status):
     keep, ptr = _bufs()
@@ -78,13 +80,19 @@ def test_error_paths_checked_on_host(case, status):
     elif case == "bad_tile":
         p.tile_q = 32
     elif case == "bad_mode":
-        mode = 3
+        mode = 4
     elif case == "null_params_sparse":
         p = None
     elif case == "nan_lambda":
         p.lambda_ = float("nan")
     elif case == "positive_lambda_fixed":
         p.lambda_, mode = 0.5, sa.MODE_FIXED
+    elif case == "mask_mode_without_mask":
+        mode = sa.MODE_MASK
+    elif case == "mask_in_other_mode":
+        p.skip_mask_in = 4096
+    elif case == "mask_mode_narrow_tile":
+        p.skip_mask_in, p.tile_q, p.tile_k, mode, D = 4096, 128, 32, sa.MODE_MASK, 128
     elif case == "bad_struct_size":
         p.struct_size = 12
     elif case == "negative_scale":
