@@ -157,11 +157,12 @@ def workload_name(cfg):
 
 
 # ---------------------------------------------------------------------------------------------- GPU arm
-def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier, sampler=None, tile_k=0):
+def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier, sampler=None, tile_k=0, mask_in=None):
     """Returns (total_ms over `steps` calls, per-call ms list, stats [B,H,2])."""
     q, k, v, out, lse, stats = bufs
     stream = torch.cuda.current_stream()
-    p = sa.make_params(lam=lam, stream=stream.cuda_stream, tile_q=cfg.tile if tile_k else 0, tile_k=tile_k)
+    p = sa.make_params(lam=lam, stream=stream.cuda_stream, tile_q=cfg.tile if tile_k else 0, tile_k=tile_k,
+                       skip_mask_in=mask_in)
     for _ in range(warmup):
         sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p, mode, stats)
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
@@ -302,17 +303,29 @@ def main():
         lam32 = math.log(P_REAL) + math.log(32 / cfg.N)       # Eq. 7 with B_c = 32
         for mname, mode, mlam, mtk in (("dense", sa.MODE_DENSE, -math.inf, 0), ("fixed", sa.MODE_FIXED, lam, 0),
                                        ("dynamic", sa.MODE_DYNAMIC, lam, 0),
-                                       ("dynamic_bc32", sa.MODE_DYNAMIC, lam32, 32)):
-            if mname.split("_")[0] not in args.modes.split(",") or (mtk and (args.no_aligned or cfg.D != 128)):
+                                       ("dynamic_bc32", sa.MODE_DYNAMIC, lam32, 32),
+                                       ("mask_replay", sa.MODE_MASK, lam, 0)):
+            if mname == "mask_replay":
+                # MASK mode fed DYNAMIC mode's own decisions: same tiles, decisions read instead of taken in the loop
+                if args.no_aligned or "dynamic" not in res:
+                    continue
+                T_dec = -(-cfg.N // cfg.tile)
+                replay_mask = torch.zeros((cfg.B, cfg.H, T_dec, T_dec), device="cuda", dtype=torch.uint8)
+                sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D,
+                                   sa.make_params(lam=lam, skip_mask_out=replay_mask,
+                                                  stream=torch.cuda.current_stream().cuda_stream), sa.MODE_DYNAMIC, stats)
+                torch.cuda.synchronize()
+            elif mname.split("_")[0] not in args.modes.split(",") or (mtk and (args.no_aligned or cfg.D != 128)):
                 continue
+            mmask = replay_mask if mname == "mask_replay" else None
             headline = (vi == 0 and mname == "dynamic")
             if headline:
                 l0 = sa.launch_count()
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk)
+                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk, mmask)
                 headline_launches = sa.launch_count() - l0 - args.warmup
                 head_total_ms = total
             else:
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk)
+                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk, mmask)
             if dist is not None:
                 t = torch.tensor([total], device="cuda")
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -343,7 +356,7 @@ def main():
                 "executed_flop_per_launch_rank0": executed_flop(BH, cfg.N, cfg.D, cfg.tile, st[None]),
                 **quality,
             }
-        for mname in ("fixed", "dynamic", "dynamic_bc32"):
+        for mname in ("fixed", "dynamic", "dynamic_bc32", "mask_replay"):
             if mname not in res or "dense" not in res:
                 continue
             if mname == "dynamic_bc32":

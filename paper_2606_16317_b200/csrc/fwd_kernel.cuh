@@ -502,6 +502,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         for (int j = 0; j < T_c; ++j) {
             PROF_TICK(0)
             if (w == 0) { TRACE(4) }
+            // MASK mode: this tile's byte is fetched before the wait for S_x(j), which hides the global-memory latency
+            bool mask_skip = false;
+            if (kSparse && mode == kModeMask) mask_skip = (j > 0) && (!grp_valid || __ldg(a.mask_in + tile_row + j) != 0);
             mbar_wait(s_full(x), sfpar);
             sfpar ^= 1u;
             tc_fence_after();
@@ -757,8 +760,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 const float ref = (mode == kModeFixed) ? m_true : lse2;
                 const float t2 = mhat2 - ref;                // Eq. 5 in log2 units (+inf at j = 0: tile 0 is kept)
                 bool row_skip = (j > 0) && (!row_valid || (t2 < lambda_log2));
-                if (mode == kModeMask)                       // decisions read from the bitmap (one byte per decision tile)
-                    row_skip = (j > 0) && (!grp_valid || __ldg(a.mask_in + tile_row + j) != 0);
+                if (mode == kModeMask) row_skip = mask_skip; // decisions read from the bitmap (one byte per decision tile)
                 const bool wskip = __all_sync(0xffffffffu, row_skip);
                 const int q = j & 3;
                 volatile int* vt = votes + (x * 4 + q) * 4;     // ring of 4 tiles (see dec)
