@@ -75,3 +75,20 @@ def test_mask_mode_reproduces_dynamic_mode_bit_for_bit(seed):
     torch.cuda.synchronize()
     assert int(st1[..., 1].sum()) > 0
     assert torch.equal(st1, st2) and torch.equal(out1.view(torch.int16), out2.view(torch.int16)) and torch.equal(lse1, lse2)
+
+
+def test_mask_mode_through_the_host_buffer_entry(seed):
+    """sparse_attn_fwd_host copies the bitmap to the device itself: same result as the device entry."""
+    rng = np.random.default_rng([seed, 77])
+    B, H, N, D, tile = 1, 2, 700, 128, 128
+    T = -(-N // tile)
+    qb, kb, vb = (f32_to_bf16_bits(rng.standard_normal((B, H, N, D), dtype=np.float32)) for _ in range(3))
+    bitmap = (rng.random((B, H, T, T)) < 0.5).astype(np.uint8)
+    o_dev, lse_dev, st_dev, _, _ = _run_mask(qb, kb, vb, bitmap, tile)
+    out = np.zeros((B, H, N, D), dtype=np.uint16)
+    lse = np.zeros((B, H, N), dtype=np.float32)
+    stats = np.zeros((B, H, 2), dtype=np.int64)
+    p = sa.make_params(lam=-3.0, skip_mask_in=bitmap)
+    sa.sparse_attn_fwd_host(qb, kb, vb, out, lse, B, H, N, D, p, sa.MODE_MASK, stats)
+    assert np.array_equal(stats, st_dev)
+    assert np.array_equal(bf16_bits_to_f64(out), o_dev) and np.array_equal(lse, lse_dev)
