@@ -1,18 +1,19 @@
 // Tile-skipping FlashAttention forward for sm_100a (B200).
 //
-// Implements SURVEY.md section 8(a) steps a1-a9 / PAPER.md section 3.1 in ONE kernel, three modes:
-// DENSE, FIXED (BLASST indicator) and DYNAMIC (DynSparse, Eq. 5-6).
+// Implements SURVEY.md section 8(a) steps a1-a9 / PAPER.md section 3.1 in ONE kernel, four modes:
+// DENSE, FIXED (BLASST indicator), DYNAMIC (DynSparse, Eq. 5-6) and MASK (decisions
+// read from a precomputed block bitmap: the block-mask methods of PAPER.md:61-62 through the same pipeline).
 //
 // CTA = 2 MMA tiles (slots X = 0, 1) of 128 query rows of one (b, h), sharing every K_j / V_j tile:
 //   warps 0-3   softmax warpgroup of slot 0 (thread <-> query row <-> TMEM lane)
 //   warps 4-7   softmax warpgroup of slot 1
 //   warp  8     TMA producer for Q (once) and the K ring (runs ahead of the decisions)
-//   warp  9     tcgen05.mma issuer of slot 0 (one elected lane) and TMEM owner
+//   warp  9     tcgen05.mma issuer of slot 0 (of both slots in DENSE mode; one elected lane) and TMEM owner
 //   warp  10    TMA producer for the V ring: slot j % NV holds V_j.  DENSE: every tile.  Sparse modes: this warp
 //               reads both slots' votes on tile j and fetches V_j only if some slot keeps tile j (plus V_{j+1}
 //               speculatively after a kept tile); an unneeded tile completes its ring phase without a load
-//   warp  11    tcgen05.mma issuer of slot 1
-// One issuer warp per slot: a thread that issues tcgen05.mma is held until its last MMA has been dispatched to the
+//   warp  11    tcgen05.mma issuer of slot 1 in the sparse modes (idle in DENSE mode)
+// One issuer warp per slot in the sparse modes: a thread that issues tcgen05.mma is held until its last MMA has been dispatched to the
 // tensor pipe, so with a single issuer every barrier wait and vote decode of one slot left the pipe idle; with two,
 // the control work of one slot overlaps the MMAs of the other.
 // TMEM (512 columns): S_0 | S_1 (fp32, BC columns each; P_X, bf16x2, aliases the first BC/2 columns of S_X)
@@ -754,7 +755,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             bool skip_grp = false, keep_any = true;
             float grp_margin = INFINITY;
             if (kSparse) {
-                // votes[x][j & 1][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
+                // votes[x][j & 3][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
                 // The MMA warp combines the four votes itself (barrier dec, one arrival per warp), so an all-skip
                 // decision reaches the tensor pipe without the four warps first synchronising with each other.
                 const float ref = (mode == kModeFixed) ? m_true : lse2;
