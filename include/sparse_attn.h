@@ -151,6 +151,21 @@ int sparse_attn_brick_permutation(int grid_t, int grid_h, int grid_w, int brick_
 int sparse_attn_reorder_tokens(const void* src, void* dst, int B, int H, int N, int D, const int32_t* perm,
                                int inverse, void* stream);
 
+/*
+ * Block mass of the dense attention probabilities (the quantity block-level Top-K / Top-P selection ranks,
+ * PAPER.md:61-62, and the "softmax ... before FA" of section 3):
+ *     mass_out[b, h, i, j] = sum over the rows r of Q tile i and the columns c of K tile j of  e^{S_rc - lse[b, h, r]}
+ * with S = softmax_scale * Q K^T and lse the DENSE log-sum-exp of row r (as sparse_attn_fwd returns it in DENSE
+ * mode), so that every row of tiles sums to the number of valid rows of Q tile i.  The Q K^T pipeline of the forward
+ * kernel without P V (one pass over all tiles, tensor cores + one ex2 per logit).
+ *   q, k     device, bf16, [B, H, N, D] contiguous, 16-byte aligned        lse   device, fp32, [B, H, N]
+ *   mass_out device, fp32, [B, H, T, T] with T = ceil(N / tile), tile = 64 (D = 64) or 128 (D = 128); overwritten
+ *   softmax_scale  0 means 1/sqrt(D);   stream  cudaStream_t, NULL = default.  Enqueues and returns.
+ * Sums are fp32 atomics: the result is reproducible to rounding, not bit for bit.
+ */
+int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float* mass_out, int B, int H, int N, int D,
+                           float softmax_scale, void* stream);
+
 /* Static string for a status code. */
 const char* sparse_attn_status_string(int status);
 

@@ -17,6 +17,7 @@ from .binding import (  # noqa: F401
     launch_count,
     library_path,
     make_params,
+    sparse_attn_block_mass,
     sparse_attn_brick_permutation,
     sparse_attn_fwd,
     sparse_attn_fwd_host,

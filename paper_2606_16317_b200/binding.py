@@ -23,6 +23,7 @@ EXPORTED_SYMBOLS = (
     "sparse_attn_fwd_host",
     "sparse_attn_lambda_from_recall",
     "sparse_attn_lambda_from_preal",
+    "sparse_attn_block_mass",
     "sparse_attn_brick_permutation",
     "sparse_attn_reorder_tokens",
     "sparse_attn_status_string",
@@ -76,6 +77,8 @@ def _load():
         lib.sparse_attn_lambda_from_recall.argtypes = [ctypes.c_double, ctypes.c_int]
         lib.sparse_attn_lambda_from_preal.restype = ctypes.c_double
         lib.sparse_attn_lambda_from_preal.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int]
+        lib.sparse_attn_block_mass.restype = ctypes.c_int
+        lib.sparse_attn_block_mass.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_int] * 4 + [ctypes.c_float, ctypes.c_void_p]
         lib.sparse_attn_brick_permutation.restype = ctypes.c_int
         lib.sparse_attn_brick_permutation.argtypes = [ctypes.c_int] * 6 + [ctypes.c_void_p]
         lib.sparse_attn_reorder_tokens.restype = ctypes.c_int
@@ -178,6 +181,15 @@ def sparse_attn_reorder_tokens(src, dst, B, H, N, D, perm, inverse, stream=None)
     """C entry point `sparse_attn_reorder_tokens` (device buffers; perm: device int32 [N])."""
     rc = _load().sparse_attn_reorder_tokens(_ptr(src), _ptr(dst), int(B), int(H), int(N), int(D), _ptr(perm),
                                             int(inverse), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_block_mass(q, k, lse, mass_out, B, H, N, D, softmax_scale=0.0, stream=None):
+    """C entry point `sparse_attn_block_mass` (device buffers): per-tile mass of the dense attention probabilities."""
+    rc = _load().sparse_attn_block_mass(_ptr(q), _ptr(k), _ptr(lse), _ptr(mass_out), int(B), int(H), int(N), int(D),
+                                        float(softmax_scale), _ptr(stream))
     if rc != 0:
         raise SparseAttnError(rc, last_error())
     return rc

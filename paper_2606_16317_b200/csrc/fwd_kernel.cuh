@@ -54,7 +54,8 @@ namespace dsa {
 #define PROF_FLUSH(base, n, cond)
 #endif
 
-enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2, kModeMask = 3 };
+enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2, kModeMask = 3,
+             kModeMass = 4 };   // internal: block mass of the dense probabilities (sparse_attn_block_mass), no P V
 
 constexpr int kNumThreads = 384;      // 3 warpgroups
 constexpr int kKProducerWarp = 8;
@@ -109,6 +110,8 @@ struct FwdArgs {
     unsigned long long* stats;   // [BH, 2] or null (pre-zeroed)
     uint8_t* skip_mask;          // [BH, T_r, T_c_dec] or null
     float* margin;               // [BH, T_r, T_c_dec] or null
+    const float* lse_in;         // MASS mode: dense lse [BH, N], natural log
+    float* mass_out;             // MASS mode: [BH, T_r, T_c] fp32, pre-zeroed: sum over the tile of e^(S - lse)
     const uint8_t* mask_in;      // MASK mode: [BH, T_r, T_c] bytes, non-zero = skip (tile 0 is kept regardless)
     int N;
     int T_r;                     // decision tiles along queries
@@ -490,6 +493,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         const bool want_margin = kDebug && a.margin != nullptr;
 
         constexpr bool kUseExpLock = DSA_EXP_LOCK == 2 || (DSA_EXP_LOCK == 1 && (kSparse ? DSA_ISSUERS_SPARSE : DSA_ISSUERS_DENSE) == 2);
+        // MASS mode: -lse_r in log2 units (+... rows beyond N contribute nothing)
+        float neg_lse2 = -INFINITY;
+        if (kSparse && mode == kModeMass && row_valid) neg_lse2 = -a.lse_in[static_cast<size_t>(bh) * a.N + grow] * kLog2e;
         float m_used = -INFINITY;   // stabiliser actually subtracted (log2 domain, may lag the true max)
         float m_true = -INFINITY;   // running max over retained tiles (log2 domain) -- FIXED mode reference
         float l = 0.f;              // sum over retained tiles of 2^(s - m_used)
@@ -532,6 +538,29 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 #pragma unroll
                 for (int c = 0; c < BC; ++c)
                     if (c >= valid_cols) su[c >> 5][c & 31] = 0xff800000u;
+            }
+            if (kSparse && SUB == 1 && mode == kModeMass) {
+                // Block mass of the dense attention probabilities: sum over the rows of this warp and the columns of the
+                // tile of e^(S_rc - lse_r) (the quantity Top-K / Top-P block selection ranks).  No P, no
+                // P V: the tile is voted "skipped", so the issuer streams Q K^T only.
+                float acc0 = 0.f, acc1 = 0.f;
+#pragma unroll
+                for (int c = 0; c < BC; c += 2) {
+                    acc0 += fast_exp2(fmaf(S_AT(c), scale_log2, neg_lse2));
+                    acc1 += fast_exp2(fmaf(S_AT(c + 1), scale_log2, neg_lse2));
+                }
+                float acc = row_valid ? acc0 + acc1 : 0.f;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                if (lane == 0 && grp_valid) atomicAdd(a.mass_out + tile_row + j, acc);
+                tc_fence_before();
+                if (lane == 0) {
+                    votes[(x * 4 + (j & 3)) * 4 + w] = (j << 2) | 1;
+                    mbar_arrive(dec(x, j & 3));
+                }
+                __syncwarp();
+                prev_skip = true;
+                continue;
             }
             float mx0 = S_AT(0), mx1 = S_AT(1), mx2 = S_AT(2), mx3 = S_AT(3);   // 4 independent 3-input max chains
 #pragma unroll
@@ -955,7 +984,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             uint32_t o[32];
             tmem_ld_x32(tO + c * 32, o);
             tmem_wait_ld();
-            if (row_valid) {
+            if (row_valid && mode != kModeMass) {          // (MASS mode has no output rows)
                 uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
 #pragma unroll
                 for (int v4 = 0; v4 < 4; ++v4) {
@@ -968,7 +997,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 }
             }
         }
-        if (a.lse && row_valid) a.lse[static_cast<size_t>(bh) * a.N + grow] = (m_used + log2f(l)) * kLn2;
+        if (a.lse && row_valid && mode != kModeMass) a.lse[static_cast<size_t>(bh) * a.N + grow] = (m_used + log2f(l)) * kLn2;
         if (a.stats && grp_leader && grp_valid) {
             atomicAdd(a.stats + 2 * bh + 0, static_cast<unsigned long long>(n_exec));
             atomicAdd(a.stats + 2 * bh + 1, static_cast<unsigned long long>(n_skip));

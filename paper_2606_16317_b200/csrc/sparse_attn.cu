@@ -294,6 +294,45 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     return 0;
 }
 
+int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float* mass_out, int B, int H, int N, int D,
+                           float softmax_scale, void* stream) {
+    g_last_error[0] = '\0';
+    if (!q || !k || !lse || !mass_out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "q, k, lse and mass_out must not be NULL");
+    if (B <= 0 || H <= 0 || N <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N must be positive (got %d, %d, %d)", B, H, N);
+    if (static_cast<long long>(B) * H > 65535) return fail(SPARSE_ATTN_ERR_SHAPE, "B*H = %lld exceeds 65535", (long long)B * H);
+    if (N > (1 << 24)) return fail(SPARSE_ATTN_ERR_SHAPE, "N = %d exceeds 2^24", N);
+    if (D != 64 && D != 128) return fail(SPARSE_ATTN_ERR_HEAD_DIM, "D = %d not in {64, 128}", D);
+    if (!(softmax_scale >= 0.f) || std::isinf(softmax_scale))
+        return fail(SPARSE_ATTN_ERR_PARAMS, "softmax_scale must be finite and >= 0 (0 = 1/sqrt(D))");
+    if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(k)) & 15u)
+        return fail(SPARSE_ATTN_ERR_ALIGNMENT, "q and k must be 16-byte aligned");
+    int rc = check_device();
+    if (rc) return rc;
+    EncodeTiledFn enc = nullptr;
+    if ((rc = get_encode_fn(&enc))) return rc;
+    const int BH = B * H;
+    const int tile = (D == 64) ? 64 : 128;
+    CUtensorMap tq, tk;
+    if ((rc = make_tmap(enc, &tq, q, BH, N, D, 128))) return rc;
+    if ((rc = make_tmap(enc, &tk, k, BH, N, D, tile))) return rc;
+    dsa::FwdArgs a;
+    std::memset(&a, 0, sizeof a);
+    a.N = N;
+    a.T_r = (N + tile - 1) / tile;
+    a.T_c = a.T_c_dec = (N + tile - 1) / tile;
+    a.n_mma_tiles = (N + 127) / 128;
+    a.mode = dsa::kModeMass;
+    a.scale_log2 = (softmax_scale > 0.f ? softmax_scale : 1.0f / std::sqrt(static_cast<float>(D))) * dsa::kLog2e;
+    a.lambda_log2 = -INFINITY;
+    a.lse_in = lse;
+    a.mass_out = mass_out;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CUDA_TRY(cudaMemsetAsync(mass_out, 0, sizeof(float) * static_cast<size_t>(BH) * a.T_r * a.T_c, st));
+    // V is never read for P V in this mode (every tile is voted skipped); the V map aliases K for the one prefetch of tile 0
+    if (D == 128) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false>(tq, tk, tk, a, BH, st);
+    return launch<64, 64, 2, 3, 2, true, false>(tq, tk, tk, a, BH, st);
+}
+
 int sparse_attn_brick_permutation(int grid_t, int grid_h, int grid_w, int brick_t, int brick_h, int brick_w,
                                   int32_t* perm_out) {
     g_last_error[0] = '\0';
