@@ -166,6 +166,21 @@ int sparse_attn_reorder_tokens(const void* src, void* dst, int B, int H, int N, 
 int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float* mass_out, int B, int H, int N, int D,
                            float softmax_scale, void* stream);
 
+/*
+ * Block selectors on a block-mass matrix (the comparison methods of PAPER.md:61-62, Table 1, Fig. 3), producing the
+ * bitmap SPARSE_ATTN_MASK consumes.  Per row of tiles (b, h, i):
+ *   SPARSE_ATTN_SELECT_TOPK  retain the ceil(param * T_c) tiles of largest mass (a fixed budget; param = kept fraction)
+ *   SPARSE_ATTN_SELECT_TOPP  retain tiles in order of decreasing mass until their share of the row's total mass reaches
+ *                            param (the tile that crosses it is retained)
+ * Equal masses are ordered by the lower tile index first; tile 0 is always retained.  param in (0, 1].
+ *   mass          device, fp32, [B, H, T_r, T_c] (sparse_attn_block_mass)     T_c <= 4096
+ *   skip_mask_out device, bytes, [B, H, T_r, T_c], 1 = skip; fully overwritten
+ * An offline analysis step (O(T_c^2) per row of tiles), enqueued on `stream`.
+ */
+enum sparse_attn_selector { SPARSE_ATTN_SELECT_TOPK = 0, SPARSE_ATTN_SELECT_TOPP = 1 };
+int sparse_attn_select_blocks(const float* mass, uint8_t* skip_mask_out, int B, int H, int T_r, int T_c, int kind,
+                              double param, void* stream);
+
 /* Static string for a status code. */
 const char* sparse_attn_status_string(int status);
 

@@ -9,6 +9,8 @@ from .binding import (  # noqa: F401
     MODE_DYNAMIC,
     MODE_FIXED,
     MODE_MASK,
+    SELECT_TOPK,
+    SELECT_TOPP,
     SparseAttnError,
     SparseAttnParams,
     lambda_from_preal,
@@ -22,6 +24,7 @@ from .binding import (  # noqa: F401
     sparse_attn_fwd,
     sparse_attn_fwd_host,
     sparse_attn_reorder_tokens,
+    sparse_attn_select_blocks,
     status_string,
     version,
 )

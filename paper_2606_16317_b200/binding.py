@@ -12,6 +12,7 @@ import os
 from typing import Optional
 
 MODE_DENSE, MODE_FIXED, MODE_DYNAMIC, MODE_MASK = 0, 1, 2, 3
+SELECT_TOPK, SELECT_TOPP = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("SPARSE_ATTN_LIB") or os.path.join(_HERE, "libsparse_attn.so")
@@ -26,6 +27,7 @@ EXPORTED_SYMBOLS = (
     "sparse_attn_block_mass",
     "sparse_attn_brick_permutation",
     "sparse_attn_reorder_tokens",
+    "sparse_attn_select_blocks",
     "sparse_attn_status_string",
     "sparse_attn_last_error",
     "sparse_attn_version",
@@ -79,6 +81,9 @@ def _load():
         lib.sparse_attn_lambda_from_preal.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int]
         lib.sparse_attn_block_mass.restype = ctypes.c_int
         lib.sparse_attn_block_mass.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_int] * 4 + [ctypes.c_float, ctypes.c_void_p]
+        lib.sparse_attn_select_blocks.restype = ctypes.c_int
+        lib.sparse_attn_select_blocks.argtypes = [ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 5 + [
+            ctypes.c_double, ctypes.c_void_p]
         lib.sparse_attn_brick_permutation.restype = ctypes.c_int
         lib.sparse_attn_brick_permutation.argtypes = [ctypes.c_int] * 6 + [ctypes.c_void_p]
         lib.sparse_attn_reorder_tokens.restype = ctypes.c_int
@@ -190,6 +195,15 @@ def sparse_attn_block_mass(q, k, lse, mass_out, B, H, N, D, softmax_scale=0.0, s
     """C entry point `sparse_attn_block_mass` (device buffers): per-tile mass of the dense attention probabilities."""
     rc = _load().sparse_attn_block_mass(_ptr(q), _ptr(k), _ptr(lse), _ptr(mass_out), int(B), int(H), int(N), int(D),
                                         float(softmax_scale), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_select_blocks(mass, skip_mask_out, B, H, T_r, T_c, kind, param, stream=None):
+    """C entry point `sparse_attn_select_blocks` (device buffers): Top-K / Top-P bitmap from a block-mass matrix."""
+    rc = _load().sparse_attn_select_blocks(_ptr(mass), _ptr(skip_mask_out), int(B), int(H), int(T_r), int(T_c), int(kind),
+                                           float(param), _ptr(stream))
     if rc != 0:
         raise SparseAttnError(rc, last_error())
     return rc

@@ -12,6 +12,7 @@
 
 #include "fwd_kernel.cuh"
 #include "reorder_kernel.cuh"
+#include "select_kernel.cuh"
 
 // K / V ring depths of the D = 128 kernels (Q 64 KB + (NK + NV) x 32 KB must fit in 227 KB)
 #ifndef DSA_NK
@@ -331,6 +332,28 @@ int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float
     // V is never read for P V in this mode (every tile is voted skipped); the V map aliases K for the one prefetch of tile 0
     if (D == 128) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false>(tq, tk, tk, a, BH, st);
     return launch<64, 64, 2, 3, 2, true, false>(tq, tk, tk, a, BH, st);
+}
+
+int sparse_attn_select_blocks(const float* mass, uint8_t* skip_mask_out, int B, int H, int T_r, int T_c, int kind,
+                              double param, void* stream) {
+    g_last_error[0] = '\0';
+    if (!mass || !skip_mask_out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "mass and skip_mask_out must not be NULL");
+    if (B <= 0 || H <= 0 || T_r <= 0 || T_c <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, T_r, T_c must be positive");
+    if (static_cast<long long>(B) * H > 65535) return fail(SPARSE_ATTN_ERR_SHAPE, "B*H = %lld exceeds 65535", (long long)B * H);
+    if (T_c > dsa::kSelectMaxTc) return fail(SPARSE_ATTN_ERR_SHAPE, "T_c = %d exceeds %d", T_c, dsa::kSelectMaxTc);
+    if (kind != SPARSE_ATTN_SELECT_TOPK && kind != SPARSE_ATTN_SELECT_TOPP)
+        return fail(SPARSE_ATTN_ERR_MODE, "kind %d not in {0 (Top-K), 1 (Top-P)}", kind);
+    if (!(param > 0.0) || param > 1.0) return fail(SPARSE_ATTN_ERR_PARAMS, "param = %g not in (0, 1]", param);
+    int rc = check_device();
+    if (rc) return rc;
+    int n_keep = static_cast<int>(std::ceil(param * T_c));
+    n_keep = std::max(1, std::min(T_c, n_keep));
+    dim3 grid(T_r, B * H, 1);
+    dsa::select_blocks_kernel<<<grid, 256, sizeof(float) * T_c, static_cast<cudaStream_t>(stream)>>>(
+        mass, skip_mask_out, T_c, kind, n_keep, param);
+    CUDA_TRY(cudaGetLastError());
+    g_reorder_launches.fetch_add(1);
+    return 0;
 }
 
 int sparse_attn_brick_permutation(int grid_t, int grid_h, int grid_w, int brick_t, int brick_h, int brick_w,

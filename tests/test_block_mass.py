@@ -56,3 +56,65 @@ def test_gpu_block_mass_matches_oracle(seed, name, N):
         ref = oracle.block_mass(bf16_bits_to_f64(qb[0, h]), bf16_bits_to_f64(kb[0, h]), tile)
         assert np.abs(got[0, h] - ref).max() < 1e-3 * tile + 1e-3 * np.abs(ref).max()
         assert np.allclose(got[0, h].sum(axis=1), ref.sum(axis=1), rtol=1e-3)
+
+
+def test_select_blocks_validates_on_host():
+    a = np.zeros(1024, dtype=np.float32)
+    b = np.zeros(1024, dtype=np.uint8)
+    cases = [((None, b, 1, 1, 4, 4, 0, 0.5), -1), ((a, None, 1, 1, 4, 4, 0, 0.5), -1), ((a, b, 1, 1, 0, 4, 0, 0.5), -2),
+             ((a, b, 1, 1, 4, 5000, 0, 0.5), -2), ((a, b, 1, 1, 4, 4, 2, 0.5), -5), ((a, b, 1, 1, 4, 4, 0, 0.0), -6),
+             ((a, b, 1, 1, 4, 4, 1, 1.5), -6)]
+    for args, status in cases:
+        with pytest.raises(sa.SparseAttnError) as e:
+            sa.sparse_attn_select_blocks(*args)
+        assert e.value.status == status, args
+    q = np.zeros(4096, dtype=np.uint16)
+    with pytest.raises(sa.SparseAttnError) as e:
+        sa.sparse_attn_block_mass(q, q, None, a, 1, 1, 16, 64)
+    assert e.value.status == -1
+    with pytest.raises(sa.SparseAttnError) as e:
+        sa.sparse_attn_block_mass(q, q, a, a, 1, 1, 16, 96)
+    assert e.value.status == -3
+
+
+@pytest.mark.gpu
+def test_gpu_selectors_match_oracle_and_drive_mask_mode(seed):
+    """Top-K / Top-P bitmaps from the GPU equal the oracle's selection on the same mass values; the bitmap then drives
+    MASK mode, whose output equals the oracle's replay of it, and Top-P's bitmap retains at least P of every row of
+    tiles' mass."""
+    cfg = CONFIGS["cfg0_aligned"]
+    qb, kb, vb = make_qkv(cfg, seed)
+    B, H, N, D, tile = cfg.B, cfg.H, cfg.N, cfg.D, cfg.tile
+    T = N // tile
+    q, k, v = (torch.from_numpy(x.view(np.int16)).cuda().view(torch.bfloat16) for x in (qb, kb, vb))
+    out = torch.empty_like(q)
+    lse = torch.empty((B, H, N), device="cuda", dtype=torch.float32)
+    sa.sparse_attn_fwd(q, k, v, out, lse, B, H, N, D, sa.make_params(), sa.MODE_DENSE, None)
+    mass = torch.empty((B, H, T, T), device="cuda", dtype=torch.float32)
+    sa.sparse_attn_block_mass(q, k, lse, mass, B, H, N, D)
+    torch.cuda.synchronize()
+    m64 = mass.cpu().numpy().astype(np.float64)
+    for kind, param, sel in ((sa.SELECT_TOPK, 0.25, oracle.select_topk), (sa.SELECT_TOPK, 0.6, oracle.select_topk),
+                             (sa.SELECT_TOPP, 0.9, oracle.select_topp), (sa.SELECT_TOPP, 0.99, oracle.select_topp)):
+        bitmap = torch.full((B, H, T, T), 255, device="cuda", dtype=torch.uint8)
+        sa.sparse_attn_select_blocks(mass, bitmap, B, H, T, T, kind, param)
+        torch.cuda.synchronize()
+        got = bitmap.cpu().numpy()
+        for h in range(H):
+            assert np.array_equal(got[0, h], sel(m64[0, h], param)), (kind, param, h)
+            if kind == sa.SELECT_TOPP:
+                kept = (m64[0, h] * (got[0, h] == 0)).sum(axis=1)
+                assert np.all(kept >= param * m64[0, h].sum(axis=1) * (1 - 1e-12))
+        stats = torch.zeros((B, H, 2), device="cuda", dtype=torch.int64)
+        lse_m = torch.empty_like(lse)
+        sa.sparse_attn_fwd(q, k, v, out, lse_m, B, H, N, D, sa.make_params(lam=-3.0, skip_mask_in=bitmap), sa.MODE_MASK, stats)
+        torch.cuda.synchronize()
+        o = bf16_bits_to_f64(out.view(torch.int16).cpu().numpy().view(np.uint16))
+        for h in range(H):
+            assert int(stats[0, h, 1]) == int(got[0, h].sum())
+            ref = oracle.run_head(qb[0, h], kb[0, h], vb[0, h], tile=tile, lam=-3.0, mode=oracle.MODE_DYNAMIC,
+                                  forced_skip=got[0, h])
+            assert np.abs(o[0, h] - ref.rows()[0]).max() < 2e-2
+        if kind == sa.SELECT_TOPP:                          # row recall >= share of the row's own tile masses kept: sanity
+            rec = torch.exp(lse_m - lse)
+            assert float(rec.mean()) > param - 0.05
