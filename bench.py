@@ -218,6 +218,46 @@ def time_reorder(sa, torch, cfg, brick, qkv, scratch_out, steps, warmup):
     return info, tuple(dst)
 
 
+def selector_comparison(sa, torch, bufs, cfg, lse_dense, out_dense, dyn, steps, warmup, barrier):
+    """the block-mask comparison methods of PAPER.md:61-62 through the same kernel.  Block mass of
+    the dense probabilities -> Top-K at DYNAMIC mode's tile budget and Top-P at DYNAMIC mode's mean recall -> MASK mode."""
+    q, k, v, out, lse, stats = bufs
+    stream = torch.cuda.current_stream()
+    T = -(-cfg.N // cfg.tile)
+    mass = torch.empty((cfg.B, cfg.H, T, T), device="cuda", dtype=torch.float32)
+    bitmap = torch.empty((cfg.B, cfg.H, T, T), device="cuda", dtype=torch.uint8)
+
+    def timed(fn, n):
+        for _ in range(2):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(n):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    ms_mass = timed(lambda: sa.sparse_attn_block_mass(q, k, lse_dense, mass, cfg.B, cfg.H, cfg.N, cfg.D, 0.0,
+                                                      stream.cuda_stream), max(3, steps // 2))
+    res = {"block_mass_ms": ms_mass,
+           "block_mass_tflops": 2.0 * cfg.B * cfg.H * cfg.N * cfg.N * cfg.D / (ms_mass * 1e-3) / 1e12,
+           "note": "mass and selection are a pre-pass the in-loop rule does not need (PAPER.md:109, :133)"}
+    for name, kind, param in (("topk_at_dynamic_budget", sa.SELECT_TOPK, max(1.0 - dyn["sparsity"], 1.0 / T)),
+                              ("topp_at_dynamic_recall", sa.SELECT_TOPP, min(max(dyn["recall_mean"], 0.01), 1.0))):
+        ms_sel = timed(lambda: sa.sparse_attn_select_blocks(mass, bitmap, cfg.B, cfg.H, T, T, kind, param,
+                                                            stream.cuda_stream), 3)
+        total, per, st = time_mode(sa, torch, bufs, cfg, sa.MODE_MASK, -math.inf, steps, warmup, barrier, None, 0, bitmap)
+        rec = torch.exp(lse - lse_dense)
+        err = (out.float() - out_dense.float()).abs()
+        res[name] = {"param": param, "select_ms": ms_sel, "attention_ms": total / steps,
+                     "sparsity": float(st[..., 1].sum() / st.sum()), "recall_min": float(rec.min()),
+                     "recall_mean": float(rec.mean()), "err_vs_dense_mean_abs": float(err.mean()),
+                     "ms_incl_prepass": total / steps + ms_mass + ms_sel}
+    return res
+
+
 def measured_hbm():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -281,6 +321,7 @@ def main():
         # SURVEY.md 8(f) NEXT-1 / PAPER.md:139: the contract workload with its tokens re-ordered into bricks
         variants.append((args.config + "_brick%dx%dx%d" % BRICK, args.config, BRICK))
     reorder_info = None
+    selectors = None
     head_total_ms = None
     sampler = ClockSampler(local_rank)
     sampler.__enter__()                     # clocks / throttle reasons are sampled inside every timed region below
@@ -373,6 +414,9 @@ def main():
                 res[mname]["decision_tile"] = "128x32"
             res[mname]["speedup_vs_dense"] = res["dense"]["ms"] / res[mname]["ms"]
             res[mname]["mma_bound_model"] = 1.0 / (1.0 - res[mname]["sparsity"] / 2.0)
+        if vi == 1 and brick is None and "dynamic" in res and "dense" in res and not args.no_aligned:
+            selectors = selector_comparison(sa, torch, bufs, vcfg, lse_dense, out_dense, res["dynamic"], args.steps,
+                                            args.warmup, barrier)
         if brick is not None and reorder_info is not None:
             for mname in ("fixed", "dynamic", "dynamic_bc32"):
                 if mname in res and "dense" in results.get(variants[0][0], {}):
@@ -462,6 +506,7 @@ def main():
                 "unit": "TFLOP/s (dense-equivalent, host buffers, H2D + kernel + D2H)",
                 "ms_per_step": e2e_s * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "token_reordering": reorder_info,
+        "block_selectors_on_aligned_workload": selectors,
         "gpu_launches": headline_launches,
         "clocks": clocks,
     }
