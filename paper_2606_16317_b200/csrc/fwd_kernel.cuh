@@ -155,6 +155,8 @@ struct SmemLayout {
 
 // kSparse = false compiles the DENSE mode only (no predicate, no vote, V always fetched);
 // kDebug adds the optional skip_mask_out / margin_out parity outputs.
+// SUB == 0: the block-mass kernel of sparse_attn_block_mass (its own instantiation, so that the forward kernels carry none
+// of its code: a run-time branch for it inside the sparse kernels cost them 7-9 %).
 // SUB > 1 (sparse modes, G = 1): the decision tile is BR x (BC / SUB) keys -- SUB decisions per MMA tile, taken in
 // ascending key order with the statistics updated after every retained one (block size 32).
 template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug, int SUB = 1>
@@ -165,7 +167,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     static_assert(D == 64 || D == 128, "head dim");
     static_assert(BC == 64 || BC == 128, "key tile");
     static_assert(2 * BC + 2 * D <= kTmemCols, "TMEM budget");
-    static_assert(SUB == 1 || (kSparse && G == 1 && (SUB == 2 || SUB == 4) && (BC / SUB) % 32 == 0), "sub-tile decisions");
+    constexpr bool kMass = SUB == 0;
+    constexpr int kSubN = SUB > 0 ? SUB : 1;
+    static_assert(SUB == 1 || (kMass && kSparse && !kDebug) ||
+                  (kSparse && G == 1 && (SUB == 2 || SUB == 4) && (BC / kSubN) % 32 == 0), "sub-tile decisions / mass kernel");
     constexpr int BR = 128 / G;
     constexpr int kSubD = D / 64;
     constexpr uint32_t kIdescQK = umma_idesc_bf16(128, BC, 0);   // S = Q K^T: A, B both K-major
@@ -344,7 +349,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int half, uint32_t mask = 0xffu) {
 #pragma unroll
                 for (int kk = half * (BC / 32); kk < (half + 1) * (BC / 32); ++kk) {
-                    if (SUB > 1 && !((mask >> (kk / (BC / 16 / SUB))) & 1u)) continue;   // P of a skipped sub-tile is never read
+                    if (SUB > 1 && !((mask >> (kk / (BC / 16 / kSubN))) & 1u)) continue;   // P of a skipped sub-tile is never read
                     // 16 keys = 16 rows of 128 B; d sub-tiles (64 columns) are L::kSubKVBytes apart (LBO)
                     umma_ts(tmem_base + 2 * BC + x * D, tmem_base + x * BC + kk * 8,
                             umma_smem_desc_sw128(vaddr + kk * 2048, L::kSubKVBytes, 1024), kIdescPV, acc || kk > 0);
@@ -495,7 +500,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         constexpr bool kUseExpLock = DSA_EXP_LOCK == 2 || (DSA_EXP_LOCK == 1 && (kSparse ? DSA_ISSUERS_SPARSE : DSA_ISSUERS_DENSE) == 2);
         // MASS mode: -lse_r in log2 units (+... rows beyond N contribute nothing)
         float neg_lse2 = -INFINITY;
-        if (kSparse && mode == kModeMass && row_valid) neg_lse2 = -a.lse_in[static_cast<size_t>(bh) * a.N + grow] * kLog2e;
+        if (kMass && row_valid) neg_lse2 = -a.lse_in[static_cast<size_t>(bh) * a.N + grow] * kLog2e;
         float m_used = -INFINITY;   // stabiliser actually subtracted (log2 domain, may lag the true max)
         float m_true = -INFINITY;   // running max over retained tiles (log2 domain) -- FIXED mode reference
         float l = 0.f;              // sum over retained tiles of 2^(s - m_used)
@@ -539,7 +544,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 for (int c = 0; c < BC; ++c)
                     if (c >= valid_cols) su[c >> 5][c & 31] = 0xff800000u;
             }
-            if (kSparse && SUB == 1 && mode == kModeMass) {
+            if constexpr (kMass) {
                 // Block mass of the dense attention probabilities: sum over the rows of this warp and the columns of the
                 // tile of e^(S_rc - lse_r) (the quantity Top-K / Top-P block selection ranks).  No P, no
                 // P V: the tile is voted "skipped", so the issuer streams Q K^T only.
@@ -984,7 +989,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             uint32_t o[32];
             tmem_ld_x32(tO + c * 32, o);
             tmem_wait_ld();
-            if (row_valid && mode != kModeMass) {          // (MASS mode has no output rows)
+            if (row_valid && !kMass) {                      // (the mass kernel has no output rows)
                 uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
 #pragma unroll
                 for (int v4 = 0; v4 < 4; ++v4) {
@@ -997,7 +1002,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 }
             }
         }
-        if (a.lse && row_valid && mode != kModeMass) a.lse[static_cast<size_t>(bh) * a.N + grow] = (m_used + log2f(l)) * kLn2;
+        if (a.lse && row_valid && !kMass) a.lse[static_cast<size_t>(bh) * a.N + grow] = (m_used + log2f(l)) * kLn2;
         if (a.stats && grp_leader && grp_valid) {
             atomicAdd(a.stats + 2 * bh + 0, static_cast<unsigned long long>(n_exec));
             atomicAdd(a.stats + 2 * bh + 1, static_cast<unsigned long long>(n_skip));

@@ -330,8 +330,8 @@ int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     CUDA_TRY(cudaMemsetAsync(mass_out, 0, sizeof(float) * static_cast<size_t>(BH) * a.T_r * a.T_c, st));
     // V is never read for P V in this mode (every tile is voted skipped); the V map aliases K for the one prefetch of tile 0
-    if (D == 128) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false>(tq, tk, tk, a, BH, st);
-    return launch<64, 64, 2, 3, 2, true, false>(tq, tk, tk, a, BH, st);
+    if (D == 128) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false, 0>(tq, tk, tk, a, BH, st);
+    return launch<64, 64, 2, 3, 2, true, false, 0>(tq, tk, tk, a, BH, st);
 }
 
 int sparse_attn_select_blocks(const float* mass, uint8_t* skip_mask_out, int B, int H, int T_r, int T_c, int kind,
