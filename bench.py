@@ -35,7 +35,7 @@ FALLBACK_TFLOPS = 1590.0
 BRICK = (4, 4, 8)       # token re-ordering brick (t, h, w): 128 tokens = one attention tile
 # dram__bytes_read.sum + dram__bytes_write.sum of one DENSE config-1 launch, ncu --set full (profiles/ncu_dense_r01.md);
 # algorithmic bytes: q + k + v + out + lse = 4 * 201.3 MB + 3.1 MB = 808 MB
-NCU_DRAM_BYTES_DENSE_CFG1 = 608.51e6 + 187.07e6
+NCU_DRAM_BYTES_DENSE_CFG1 = 610.71e6 + 189.00e6
 
 
 def measured_peaks():
