@@ -17,25 +17,28 @@ MODE_DENSE, MODE_FIXED, MODE_DYNAMIC = 0, 1, 2
 
 
 def brute_force_head(q: np.ndarray, k: np.ndarray, v: np.ndarray, *, tile: int, lam: float, mode: int,
-                     scale: Optional[float] = None):
-    """q, k, v: float64 [N, D] (already widened from bf16).
+                     scale: Optional[float] = None, tile_k: Optional[int] = None):
+    """q, k, v: float64 [N, D] (already widened from bf16).  Decision tiles are `tile` query rows by
+    `tile_k` keys (default: square; the paper gives B_c only -- 128 for 14B, 32 for 5B).
 
     Returns dict(out [N, D], lse [N], skip [T_r, T_c] uint8, margin [T_r, T_c]).
     """
     N, D = q.shape
     if scale is None:
         scale = 1.0 / math.sqrt(D)
-    T = -(-N // tile)
+    width = tile if tile_k is None else tile_k
+    T_r = -(-N // tile)
+    T_c = -(-N // width)
     S = scale * (q @ k.T)                               # logits, S includes the scale
     out = np.zeros((N, D))
     lse = np.zeros(N)
-    skip = np.zeros((T, T), dtype=np.uint8)
-    margin = np.full((T, T), np.inf)
-    for i in range(T):
+    skip = np.zeros((T_r, T_c), dtype=np.uint8)
+    margin = np.full((T_r, T_c), np.inf)
+    for i in range(T_r):
         rows = range(i * tile, min(N, (i + 1) * tile))
         retained_cols = []                              # explicit set: columns of tiles k notin J_i
-        for j in range(T):
-            cols = list(range(j * tile, min(N, (j + 1) * tile)))
+        for j in range(T_c):
+            cols = list(range(j * width, min(N, (j + 1) * width)))
             if mode == MODE_DENSE or not retained_cols:
                 keep = True                             # first tile: LSE^(0) = -inf, t = +inf
             else:

@@ -27,7 +27,8 @@
  * fused or reordered.  Inputs are bf16 bit patterns, widened exactly to fp64.
  *
  * Pins (tests/test_oracle_pins.py): P1 dense == textbook softmax / torch fp64 SDPA; P2/P3 recall
- * bound; P4 counts; P5 Eq. 1 identity; P6 DYNAMIC superset of FIXED; P7-P9 closed forms; P10 brute force.
+ * bound; P4 counts; P5 Eq. 1 identity; P6 DYNAMIC superset of FIXED; P7-P9 closed forms; P10 brute force --
+ * P7-P10 also with rectangular decision tiles (tile_k != tile_q: 128 x 32, 128 x 64, 64 x 16).
  * Parity unpinned: the absolute sparsity reached on any input (the paper's 61-82 % are on Wan 2.2
  * activations, which are not available).
  */

@@ -176,6 +176,32 @@ def test_p7_uniform_logits_closed_form(lam, kept):
     np.testing.assert_allclose(lse, math.log(kept * tile), atol=1e-12)
 
 
+@pytest.mark.parametrize("lam", [-6.0, -5.0, -4.0, -8.0])
+def test_p7_uniform_logits_rectangular_tiles(lam):
+    """P7 with decision tiles of 128 rows x 32 keys ("block size 32"): with all logits
+    equal, DYNAMIC keeps exactly floor(e^-lambda / 32) + 1 leading 32-key tiles.  A slip that takes T_c, the column
+    offset or the tile width from tile_q instead of tile_k fails here."""
+    N, D, tq, tk = 1024, 64, 128, 32
+    T_r, T_c = N // tq, N // tk
+    kept = min(T_c, int(math.floor(math.exp(-lam) / tk)) + 1)
+    assert {-6.0: 13, -5.0: 5, -4.0: 2, -8.0: 32}[lam] == kept
+    qb = np.zeros((N, D), dtype=np.uint16)
+    rng = np.random.default_rng(5)
+    kb = f32_to_bf16_bits(rng.standard_normal((N, D)).astype(np.float32))
+    vb = f32_to_bf16_bits(rng.standard_normal((N, D)).astype(np.float32))
+    dyn = oracle.run_head(qb, kb, vb, tile=tq, tile_k=tk, lam=lam, mode=MODE_DYNAMIC)
+    assert dyn.skip.shape == (T_r, T_c)
+    expect = np.zeros((T_r, T_c), dtype=np.uint8)
+    expect[:, kept:] = 1
+    np.testing.assert_array_equal(dyn.skip, expect)
+    fix = oracle.run_head(qb, kb, vb, tile=tq, tile_k=tk, lam=lam, mode=MODE_FIXED)
+    assert fix.skipped == 0
+    o, lse = dyn.rows()
+    v = bf16_bits_to_f64(vb)
+    np.testing.assert_allclose(o, np.broadcast_to(v[:kept * tk].mean(axis=0), o.shape), atol=1e-12)
+    np.testing.assert_allclose(lse, math.log(kept * tk), atol=1e-12)
+
+
 def _winner_inputs(N, D, tile, winner_col, W):
     """Each row has logit W at column `winner_col` and 0 elsewhere (scale 1/sqrt(D))."""
     a = math.sqrt(W * math.sqrt(D))
@@ -218,7 +244,63 @@ def test_p9_late_winner():
     np.testing.assert_allclose(dyn.rows()[1], math.log(kstar * tile + math.exp(W) + tile - 1), atol=1e-12)
 
 
+@pytest.mark.parametrize("tq,tk", [(128, 32), (128, 64), (64, 16)])
+def test_p8_p9_winner_rectangular_tiles(tq, tk):
+    """P8 / P9 with tile_k != tile_q: the winner sits in the FIRST (col 5) or the LAST tile_k-wide decision tile."""
+    N, D, lam, W = 1024, 64, -6.0, 8.0
+    T_r, T_c = N // tq, N // tk
+    kstar = int(math.floor(math.exp(-lam) / tk)) + 1
+    # early winner: every decision tile after the first is skipped in both modes
+    qb, kb, vb = _winner_inputs(N, D, tq, winner_col=5, W=W)
+    for mode in (MODE_DYNAMIC, MODE_FIXED):
+        res = oracle.run_head(qb, kb, vb, tile=tq, tile_k=tk, lam=lam, mode=mode)
+        expect = np.ones((T_r, T_c), dtype=np.uint8)
+        expect[:, 0] = 0
+        np.testing.assert_array_equal(res.skip, expect)
+        np.testing.assert_allclose(res.rows()[1], math.log(math.exp(W) + tk - 1), atol=1e-12)
+    # late winner, in the last tile_k keys: FIXED skips nothing; DYNAMIC skips the dilution tiles, keeps the winner tile
+    qb, kb, vb = _winner_inputs(N, D, tq, winner_col=N - 3, W=W)
+    fix = oracle.run_head(qb, kb, vb, tile=tq, tile_k=tk, lam=lam, mode=MODE_FIXED)
+    assert fix.skipped == 0
+    dyn = oracle.run_head(qb, kb, vb, tile=tq, tile_k=tk, lam=lam, mode=MODE_DYNAMIC)
+    expect = np.zeros((T_r, T_c), dtype=np.uint8)
+    expect[:, kstar:T_c - 1] = 1
+    np.testing.assert_array_equal(dyn.skip, expect)
+    np.testing.assert_allclose(dyn.rows()[1], math.log(kstar * tk + math.exp(W) + tk - 1), atol=1e-12)
+
+
 # ---------------------------------------------------------------- P10: brute force on tiny inputs
+@pytest.mark.parametrize("N,D,tq,tk", [(330, 32, 128, 32), (200, 64, 128, 64), (150, 16, 64, 16), (257, 32, 128, 32)])
+@pytest.mark.parametrize("mode", [MODE_DYNAMIC, MODE_FIXED])
+def test_p10_brute_force_rectangular_tiles(N, D, tq, tk, mode, seed):
+    """P10 with tile_k != tile_q (ragged N in both directions): the independent formulation takes its own tile_q /
+    tile_k, so the streaming oracle's rectangular-tile regime (every 128 x 64 / 128 x 32 parity claim rests on it) is
+    pinned like the square one."""
+    rng = np.random.default_rng([seed, N, D, tq, tk, mode])
+    qb, kb, vb = _rand_bits(rng, N, D, 1.8)
+    q, k, v = (bf16_bits_to_f64(x) for x in (qb, kb, vb))
+    T_r, T_c = -(-N // tq), -(-N // tk)
+    probe = oracle.run_head(qb, kb, vb, tile=tq, tile_k=tk, lam=0.0, mode=mode, forced_skip=np.zeros((T_r, T_c), dtype=np.uint8))
+    assert probe.skip.shape == (T_r, T_c)
+    finite = probe.margin[np.isfinite(probe.margin)]
+    n_skip_total = 0
+    for lam in np.quantile(finite, [0.2, 0.5, 0.8]):
+        lam = float(lam)
+        res = oracle.run_head(qb, kb, vb, tile=tq, tile_k=tk, lam=lam, mode=mode)
+        bf = oracle.brute_force_head(q, k, v, tile=tq, tile_k=tk, lam=lam, mode=mode)
+        assert bf["skip"].shape == (T_r, T_c)
+        safe = ~(np.abs(bf["margin"]) < 1e-9)
+        np.testing.assert_array_equal(res.skip[safe], bf["skip"][safe])
+        if np.array_equal(res.skip, bf["skip"]):
+            o, lse = res.rows()
+            np.testing.assert_allclose(o, bf["out"], rtol=0, atol=1e-11)
+            np.testing.assert_allclose(lse, bf["lse"], rtol=0, atol=1e-11)
+            fin = np.isfinite(bf["margin"])
+            np.testing.assert_allclose(res.margin[fin], bf["margin"][fin], rtol=0, atol=1e-11)
+        n_skip_total += res.skipped
+    assert n_skip_total > 0
+
+
 @pytest.mark.parametrize("N,D,tile", [(256, 64, 64), (200, 64, 64), (130, 32, 32), (384, 128, 128), (97, 16, 16)])
 @pytest.mark.parametrize("mode", [MODE_DYNAMIC, MODE_FIXED])
 def test_p10_brute_force_equals_streaming(N, D, tile, mode, seed):
