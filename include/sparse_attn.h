@@ -44,8 +44,8 @@ enum sparse_attn_status {
     SPARSE_ATTN_ERR_TILE = -4,         /* tile_q / tile_k not a supported decision tile for this D and mode */
     SPARSE_ATTN_ERR_MODE = -5,         /* mode not in {0, 1, 2, 3} */
     SPARSE_ATTN_ERR_PARAMS = -6,       /* params NULL in a sparse mode, struct_size wrong, lambda NaN,
-                                          lambda > 0 in FIXED mode, softmax_scale negative / non-finite,
-                                          skip_mask_in NULL in MASK mode or set in another mode */
+                                          lambda > 0 in FIXED mode or with tile_k < 128 at D = 128, softmax_scale
+                                          negative / non-finite, skip_mask_in NULL in MASK mode or set in another mode */
     SPARSE_ATTN_ERR_ALIGNMENT = -7,    /* q, k, v or out not 16-byte aligned (TMA / vector stores) */
     SPARSE_ATTN_ERR_DEVICE = -8,       /* no CUDA device, or the current device is not sm_100 (B200) */
     SPARSE_ATTN_ERR_CUDA = -9          /* a CUDA runtime / driver call failed; see sparse_attn_last_error() */
@@ -65,7 +65,9 @@ typedef struct sparse_attn_params {
                                D = 128 also accepts tile_q = 128 with tile_k = 64 or 32 in the sparse modes ("block
                                size 32"): the decision tiles of 64 / 32 keys are visited in ascending
                                key order, the statistics are updated after every retained one, and exp, row sum and
-                               P V are skipped per decision tile.  T_c below is then ceil(N / tile_k). */
+                               P V are skipped per decision tile.  T_c below is then ceil(N / tile_k).  With these
+                               narrow tiles lambda must be <= 0 (the softmax stabiliser follows the max of the whole
+                               128-key MMA tile, which only a non-positive threshold is certain to retain). */
     void* stream;           /* cudaStream_t to launch on; NULL = the default stream */
     uint8_t* skip_mask_out; /* optional, device, [B, H, T_r, T_c] bytes, 1 = tile skipped, fully overwritten.
                                T_r = ceil(N / tile_q), T_c = ceil(N / tile_k).  NULL in timed runs. */
@@ -102,10 +104,13 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
                     const sparse_attn_params* params, int mode, int64_t* stats_out);
 
 /*
- * Same operation with HOST buffers (pageable or pinned): allocates device scratch, copies q, k, v
- * host->device, runs sparse_attn_fwd, copies out / lse / stats back, synchronises and frees.
- * params->skip_mask_out / margin_out, if set, are host pointers here too.  Used for end-to-end
- * timing; layouts as above.
+ * Same operation with HOST buffers (pinned for full speed; pageable works, without overlap): takes
+ * device scratch from the stream-ordered pool, cuts the B*H heads (independent units) into up to 8
+ * chunks and pipelines them over internal streams -- the host->device copy of chunk c+1 and the
+ * device->host copy of chunk c-1 run under the kernel of chunk c -- then synchronises and frees.
+ * params->skip_mask_out / margin_out / skip_mask_in, if set, are host pointers here too; work is
+ * ordered after whatever is already enqueued on params->stream.  Used for end-to-end timing;
+ * layouts as above.  Synchronous: on return every output buffer is complete.
  */
 int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse,
                          int B, int H, int N, int D,
@@ -167,6 +172,15 @@ int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float
                            float softmax_scale, void* stream);
 
 /*
+ * sparse_attn_block_mass plus the per-tile sum of SQUARED probabilities, the other ingredient of the error-variance
+ * bound of Eq. 2-3 (Var(E) = sigma^2 [sum_S p_j^2 + (S_1/(1-S_1))^2 sum_K p_j^2]):
+ *     sqmass_out[b, h, i, j] = sum over the rows r of Q tile i and the columns c of K tile j of  e^{2 (S_rc - lse[b, h, r])}
+ * Same pass, same layout and arguments as sparse_attn_block_mass; sqmass_out may be NULL (then identical to it).
+ */
+int sparse_attn_block_stats(const void* q, const void* k, const float* lse, float* mass_out, float* sqmass_out,
+                            int B, int H, int N, int D, float softmax_scale, void* stream);
+
+/*
  * Block selectors on a block-mass matrix (the comparison methods of PAPER.md:61-62, Table 1, Fig. 3), producing the
  * bitmap SPARSE_ATTN_MASK consumes.  Per row of tiles (b, h, i):
  *   SPARSE_ATTN_SELECT_TOPK  retain the ceil(param * T_c) tiles of largest mass (a fixed budget; param = kept fraction)
@@ -180,6 +194,24 @@ int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float
 enum sparse_attn_selector { SPARSE_ATTN_SELECT_TOPK = 0, SPARSE_ATTN_SELECT_TOPP = 1 };
 int sparse_attn_select_blocks(const float* mass, uint8_t* skip_mask_out, int B, int H, int T_r, int T_c, int kind,
                               double param, void* stream);
+
+/*
+ * The "ideal" mask of PAPER.md section 3 (lines 105-109) at block level, for SPARSE_ATTN_MASK: "Given an upper
+ * tolerance limit for the error variance Theta ... sort P_j in ascending order ... sequentially move the smallest
+ * p_j from K to S ... stop when the condition represented by Eq. 3 is met".  Per row of tiles (b, h, i), with
+ * P_j = mass[i, j] / rows_i and q_j = sqmass[i, j] / rows_i (block sums averaged over the rows_i valid rows of Q tile i):
+ * tiles j >= 1 are discarded in order of increasing mass (equal masses: lower index first) for as long as
+ *     sum_{S} q_j + (S_1 / (1 - S_1))^2 * sum_{K} q_j <= theta,        S_1 = sum_{S} P_j            (Eq. 3)
+ * holds with the tile included in S; the scan stops at the first tile that would violate it.  Tile 0 is never a
+ * candidate (MASK mode retains it regardless).  theta = 0 discards only tiles of zero mass.
+ *   mass, sqmass   device, fp32, [B, H, T_r, T_c] (sparse_attn_block_stats);  T_r = ceil(N / tile_q), T_c <= 4096
+ *   skip_mask_out  device, bytes, [B, H, T_r, T_c], 1 = skip; fully overwritten
+ *   N, tile_q      tokens and decision-tile rows (64 or 128): rows_i = min(tile_q, N - i * tile_q)
+ * "Requires softmax computation, sorting, and dynamic decision-making before FA": an offline
+ * comparison method, O(T_c^2) per row of tiles, enqueued on `stream`.
+ */
+int sparse_attn_select_blocks_greedy(const float* mass, const float* sqmass, uint8_t* skip_mask_out, int B, int H, int N,
+                                     int tile_q, int T_c, double theta, void* stream);
 
 /* Static string for a status code. */
 const char* sparse_attn_status_string(int status);

@@ -20,11 +20,13 @@ from .binding import (  # noqa: F401
     library_path,
     make_params,
     sparse_attn_block_mass,
+    sparse_attn_block_stats,
     sparse_attn_brick_permutation,
     sparse_attn_fwd,
     sparse_attn_fwd_host,
     sparse_attn_reorder_tokens,
     sparse_attn_select_blocks,
+    sparse_attn_select_blocks_greedy,
     status_string,
     version,
 )

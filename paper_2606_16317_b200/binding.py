@@ -25,6 +25,8 @@ EXPORTED_SYMBOLS = (
     "sparse_attn_lambda_from_recall",
     "sparse_attn_lambda_from_preal",
     "sparse_attn_block_mass",
+    "sparse_attn_block_stats",
+    "sparse_attn_select_blocks_greedy",
     "sparse_attn_brick_permutation",
     "sparse_attn_reorder_tokens",
     "sparse_attn_select_blocks",
@@ -81,6 +83,10 @@ def _load():
         lib.sparse_attn_lambda_from_preal.argtypes = [ctypes.c_double, ctypes.c_int, ctypes.c_int]
         lib.sparse_attn_block_mass.restype = ctypes.c_int
         lib.sparse_attn_block_mass.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_int] * 4 + [ctypes.c_float, ctypes.c_void_p]
+        lib.sparse_attn_block_stats.restype = ctypes.c_int
+        lib.sparse_attn_block_stats.argtypes = [ctypes.c_void_p] * 5 + [ctypes.c_int] * 4 + [ctypes.c_float, ctypes.c_void_p]
+        lib.sparse_attn_select_blocks_greedy.restype = ctypes.c_int
+        lib.sparse_attn_select_blocks_greedy.argtypes = [ctypes.c_void_p] * 3 + [ctypes.c_int] * 5 + [ctypes.c_double, ctypes.c_void_p]
         lib.sparse_attn_select_blocks.restype = ctypes.c_int
         lib.sparse_attn_select_blocks.argtypes = [ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 5 + [
             ctypes.c_double, ctypes.c_void_p]
@@ -195,6 +201,24 @@ def sparse_attn_block_mass(q, k, lse, mass_out, B, H, N, D, softmax_scale=0.0, s
     """C entry point `sparse_attn_block_mass` (device buffers): per-tile mass of the dense attention probabilities."""
     rc = _load().sparse_attn_block_mass(_ptr(q), _ptr(k), _ptr(lse), _ptr(mass_out), int(B), int(H), int(N), int(D),
                                         float(softmax_scale), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_block_stats(q, k, lse, mass_out, sqmass_out, B, H, N, D, softmax_scale=0.0, stream=None):
+    """C entry point `sparse_attn_block_stats` (device buffers): per-tile sums of p and of p^2 of the dense probabilities."""
+    rc = _load().sparse_attn_block_stats(_ptr(q), _ptr(k), _ptr(lse), _ptr(mass_out), _ptr(sqmass_out), int(B), int(H), int(N),
+                                         int(D), float(softmax_scale), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_select_blocks_greedy(mass, sqmass, skip_mask_out, B, H, N, tile_q, T_c, theta, stream=None):
+    """C entry point `sparse_attn_select_blocks_greedy` (device buffers): the section-3 mask under Eq. 3's bound."""
+    rc = _load().sparse_attn_select_blocks_greedy(_ptr(mass), _ptr(sqmass), _ptr(skip_mask_out), int(B), int(H), int(N),
+                                                  int(tile_q), int(T_c), float(theta), _ptr(stream))
     if rc != 0:
         raise SparseAttnError(rc, last_error())
     return rc

@@ -13,9 +13,9 @@
 //               reads both slots' votes on tile j and fetches V_j only if some slot keeps tile j (plus V_{j+1}
 //               speculatively after a kept tile); an unneeded tile completes its ring phase without a load
 //   warp  11    tcgen05.mma issuer of slot 1 in the sparse modes (idle in DENSE mode)
-// One issuer warp per slot in the sparse modes: a thread that issues tcgen05.mma is held until its last MMA has been dispatched to the
-// tensor pipe, so with a single issuer every barrier wait and vote decode of one slot left the pipe idle; with two,
-// the control work of one slot overlaps the MMAs of the other.
+// One issuer warp per slot in the sparse modes: a thread that issues tcgen05.mma is held until its last MMA has been
+// dispatched to the tensor pipe, so with a single issuer every barrier wait and vote decode of one slot left the pipe
+// idle; with two, the control work of one slot overlaps the MMAs of the other.
 // TMEM (512 columns): S_0 | S_1 (fp32, BC columns each; P_X, bf16x2, aliases the first BC/2 columns of S_X)
 //                     O_0 | O_1 (fp32, D columns each).
 // Per slot X and K tile j:  S_X = Q_X K_j^T (always)  ->  softmax warpgroup: row max, skip predicate,
@@ -30,30 +30,6 @@
 
 namespace dsa {
 
-#ifdef DSA_PROF
-#if DSA_PROF == 2   // timeline of CTA (0, 0) only, no per-phase accumulators
-#define PROF_DECL(n)
-#define PROF_TICK(i)
-#define PROF_FLUSH(base, n, cond)
-#else
-#define PROF_DECL(n) unsigned long long prof_acc[n] = {}; long long prof_t = clock64();
-#define PROF_TICK(i) { long long t__ = clock64(); prof_acc[i] += t__ - prof_t; prof_t = t__; }
-#define PROF_FLUSH(base, n, cond) if (a.prof && (cond)) { for (int i__ = 0; i__ < n; ++i__) a.prof[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * 32 + base + i__] = prof_acc[i__]; }
-#endif
-#define TRACE(slot) if (a.prof && blockIdx.x == DSA_TRACE_CTA && blockIdx.y == 0 && j >= DSA_TRACE_J0 && j < DSA_TRACE_J0 + 32 && (threadIdx.x & 31) == 0) a.prof[(1 << 20) + ((j - DSA_TRACE_J0) * 2 + x) * 32 + (slot)] = clock64();
-#ifndef DSA_TRACE_CTA
-#define DSA_TRACE_CTA 0
-#endif
-#ifndef DSA_TRACE_J0
-#define DSA_TRACE_J0 0
-#endif
-#else
-#define TRACE(slot)
-#define PROF_DECL(n)
-#define PROF_TICK(i)
-#define PROF_FLUSH(base, n, cond)
-#endif
-
 enum : int { kModeDense = 0, kModeFixed = 1, kModeDynamic = 2, kModeMask = 3,
              kModeMass = 4 };   // internal: block mass of the dense probabilities (sparse_attn_block_mass), no P V
 
@@ -65,44 +41,23 @@ constexpr int kMmaWarp1 = 11;
 // setmaxnreg: the kernel launches with 168 registers/thread (65536 / 384); the two softmax warpgroups grow to
 // 208 (a full S row lives in registers), the producer/MMA warpgroup shrinks to 88.  The registers the 128
 // threads give up must cover what the 256 softmax threads take, or setmaxnreg.inc never returns.
-#ifndef DSA_REGS_SOFTMAX
-#define DSA_REGS_SOFTMAX 208
-#define DSA_REGS_OTHER 88
-#endif
 constexpr int kRegsLaunch = 168;
-constexpr int kRegsSoftmax = DSA_REGS_SOFTMAX;
-constexpr int kRegsOther = DSA_REGS_OTHER;
+constexpr int kRegsSoftmax = 208;
+constexpr int kRegsOther = 88;
 static_assert((kRegsLaunch - kRegsOther) * 128 >= (kRegsSoftmax - kRegsLaunch) * 256, "setmaxnreg pool imbalance");
 constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 // lazy rescale: O and l are only rescaled when the row max grew by more than 2^8 (log2 domain).
 constexpr float kRescaleThreshold = 8.0f;
-// Early issue of the second half of S_x(j+1) (keys [BC/2, BC), columns P_x(j) does not use) as soon as S_x(j) is in
-// registers.  Measured slower on B200 (dense cfg1 11.3 ms against 10.1 ms): with A = Q_x read from shared memory every
-// N = BC/2 instruction still reads the whole 4 KB A tile, so two half-width Q K^T cost ~1.5x one full-width one.  Off.
-#ifndef DSA_EARLY_B
-#define DSA_EARLY_B 0
+// Of every 16 pairs of logits (one 32-column chunk), this many take their exponential on the FMA pipe (range
+// reduction + cubic, packed f32x2) instead of MUFU.EX2: the MUFU pipe (16 / clk / SM) needs exactly as long for the
+// N^2 exponentials as the tensor pipe for the MMAs, so every exponential moved off it shortens the softmax phase.
+#ifndef DSA_POLY_PAIRS
+#define DSA_POLY_PAIRS 0
 #endif
-#ifndef DSA_F32X2
-#define DSA_F32X2 1
-#endif
-#ifndef DSA_EXP
-#define DSA_EXP 0   // timing experiments only (results are wrong unless nothing is skipped)
-#endif
-#ifndef DSA_EXP_LOCK
-#define DSA_EXP_LOCK 0
-#endif
-// number of tcgen05.mma issuer warps (1: warp 9 drives both slots; 2: one warp per slot)
-#ifndef DSA_GATE
-#define DSA_GATE 1
-#endif
-#ifndef DSA_ISSUERS_DENSE
-#define DSA_ISSUERS_DENSE 1
-#endif
-#ifndef DSA_ISSUERS_SPARSE
-#define DSA_ISSUERS_SPARSE 2
-#endif
+constexpr int kPolyPairs = DSA_POLY_PAIRS;
+static_assert(kPolyPairs == 0 || kPolyPairs == 1 || kPolyPairs == 2 || kPolyPairs == 4 || kPolyPairs == 8 || kPolyPairs == 16, "pairs per chunk on the FMA pipe");
 
 struct FwdArgs {
     __nv_bfloat16* out;          // [BH, N, D]
@@ -112,6 +67,7 @@ struct FwdArgs {
     float* margin;               // [BH, T_r, T_c_dec] or null
     const float* lse_in;         // MASS mode: dense lse [BH, N], natural log
     float* mass_out;             // MASS mode: [BH, T_r, T_c] fp32, pre-zeroed: sum over the tile of e^(S - lse)
+    float* sqmass_out;           // MASS mode: optional [BH, T_r, T_c] fp32, pre-zeroed: sum over the tile of e^(2 (S - lse))
     const uint8_t* mask_in;      // MASK mode: [BH, T_r, T_c] bytes, non-zero = skip (tile 0 is kept regardless)
     int N;
     int T_r;                     // decision tiles along queries
@@ -121,9 +77,6 @@ struct FwdArgs {
     int mode;
     float scale_log2;            // softmax_scale * log2(e)
     float lambda_log2;           // lambda * log2(e)
-#ifdef DSA_PROF
-    unsigned long long* prof;    // [n_cta][32] cycle counters (profiling builds only)
-#endif
 };
 
 template <int D, int BC, int NK, int NV>
@@ -136,22 +89,69 @@ struct SmemLayout {
     static constexpr int kKOff = 2 * kQSlotBytes;
     static constexpr int kVOff = kKOff + NK * kKVStageBytes;
     static constexpr int kBarOff = kVOff + NV * kKVStageBytes;
-    // barriers (8 B each): q_full[2] k_full[NK] k_empty[NK] v_full[NV] v_empty[NV]
-    //                      s_full[2] p_half[2] p_ready[2] o_full[2] s_read[2] dec[2][4]
-    static constexpr int kNumBars = 2 + 2 * NK + 2 * NV + 8 + 2 + 8;
-    static constexpr int kMiscOff = kBarOff + 8 * kNumBars;
-    // misc: tmem_ptr (4) | pad (12) | votes[2][4][4] (128) | wmax[2][4][4] (128) | in_exp[2][4] (32) | prog[2] (16) | pvmask[2][4] (32)
-    static constexpr int kVotesOff = kMiscOff + 16;
-    static constexpr int kLockOff = kVotesOff + 256;
-    static constexpr int kProgOff = kLockOff + 32;
-    static constexpr int kPvMaskOff = kProgOff + 16;       // pvmask[2][4]: kept sub-tiles of tile j (SUB > 1), ring like votes
-    static constexpr int kPreOff = kPvMaskOff + 32;        // pre[2][4][4]: per-warp votes on sub-tiles (SUB > 1): buffers 0, 1
-                                                           // preliminary round of tile j (by parity), 2, 3 later rounds
-    static constexpr int kMiscBytes = 16 + 128 + 128 + 32 + 16 + 32 + 128;
-    static constexpr int kTotal = kMiscOff + kMiscBytes;
+    // CTA-wide barriers (8 B each): q_full[2] k_full[NK] k_empty[NK] v_full[NV] v_empty[NV]
+    static constexpr int kNumCtaBars = 2 + 2 * NK + 2 * NV;
+    static constexpr int kMiscOff = kBarOff + 8 * kNumCtaBars;          // tmem_ptr (4) | pad (4) | prog[2] (8)
+    // Per-slot block: everything one softmax warpgroup and its issuer exchange sits at a constant offset from ONE
+    // base address per slot, which the softmax threads keep in a register for the whole K loop.
+    static constexpr int kSlotOff = kMiscOff + 16;
+    static constexpr int kSFull = 0;        // S_X(j) complete in TMEM                                  (count 1)
+    static constexpr int kPHalf = 8;        // first half of P_X written (kept tiles only)             (count 128)
+    static constexpr int kPReady = 16;      // all of P_X written (kept tiles only)                    (count 128)
+    static constexpr int kOFull = 24;       // last P V of slot X complete                             (count 1)
+    static constexpr int kSRead = 32;       // the 4 warps of slot X hold S_X(j) in registers          (count 4)
+    static constexpr int kDec = 48;         // dec[4]: the 4 warps of slot X have voted on tile j      (count 4), ring j & 3
+    static constexpr int kVotes = 80;       // votes[4][4]: (j << 2) | vote of warp w on tile j, ring j & 3, 16-B rows
+    static constexpr int kWmax = 144;       // wmax[4][4]: per-warp max of t (debug margins), ring j & 3
+    static constexpr int kPvMask = 208;     // pvmask[4]: kept sub-tiles of tile j (SUB > 1), ring j & 3
+    static constexpr int kPre = 224;        // pre[5][4] (SUB > 1): per-warp sub-tile votes: groups 0, 1 the preliminary
+                                            // round of tile j (by parity), groups 2..4 the later rounds of sub-tiles 1..3
+    static constexpr int kSlotStride = 304;
+    static constexpr int kTotal = kSlotOff + 2 * kSlotStride;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
+    static_assert(kSlotOff % 16 == 0 && kSlotStride % 16 == 0, "vote rows are read with 16-byte loads");
     static_assert(kDynamicBytes <= 232448, "exceeds the 227 KB of shared memory a CTA may use");
 };
+
+// 2^x for two logits on the FMA pipe (the MUFU-free path of the exp phase): x = n + f with n = round(x) taken from
+// the low mantissa bits of x + 1.5 * 2^23, 2^f by a cubic (minimax on [-0.5, 0.5], relative error 7.5e-5: below the
+// 2^-9 of the bf16 rounding of P that follows), 2^n by adding n to the exponent field.  x is clamped to >= -126.
+__device__ __forceinline__ void exp2_poly_x2(uint64_t X, float& p0, float& p1) {
+    float x0, x1;
+    unpack_f32x2(X, x0, x1);
+    const uint64_t Xc = pack_f32x2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+    const uint64_t T = add_f32x2(Xc, pack_f32x2(12582912.f, 12582912.f));
+    const uint64_t Nf = add_f32x2(T, pack_f32x2(-12582912.f, -12582912.f));
+    const uint64_t F = fma_f32x2(Nf, pack_f32x2(-1.f, -1.f), Xc);
+    uint64_t P = fma_f32x2(pack_f32x2(0.05517167f, 0.05517167f), F, pack_f32x2(0.24261114f, 0.24261114f));
+    P = fma_f32x2(P, F, pack_f32x2(0.69326097f, 0.69326097f));
+    P = fma_f32x2(P, F, pack_f32x2(0.99992806f, 0.99992806f));
+    float f0, f1, t0, t1;
+    unpack_f32x2(P, f0, f1);
+    unpack_f32x2(T, t0, t1);
+    p0 = __int_as_float(__float_as_int(f0) + (__float_as_int(t0) << 23));
+    p1 = __int_as_float(__float_as_int(f1) + (__float_as_int(t1) << 23));
+}
+
+// a5 for 32 columns of one row: P = 2^(s * scale - m) -> 16 packed bf16x2, row sum into the packed pair rs2.
+__device__ __forceinline__ void exp_chunk(const uint32_t (&s)[32], uint64_t scale2, uint64_t negm2, uint64_t& rs2,
+                                          uint32_t (&pk)[16]) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        const uint64_t X = fma_f32x2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), scale2, negm2);
+        float p0, p1;
+        if (kPolyPairs > 0 && (i % (16 / (kPolyPairs > 0 ? kPolyPairs : 1))) == (16 / (kPolyPairs > 0 ? kPolyPairs : 1)) - 1) {
+            exp2_poly_x2(X, p0, p1);
+        } else {
+            float x0, x1;
+            unpack_f32x2(X, x0, x1);
+            p0 = fast_exp2(x0);
+            p1 = fast_exp2(x1);
+        }
+        rs2 = add_f32x2(rs2, pack_f32x2(p0, p1));
+        pk[i] = pack_bf16x2(p0, p1);
+    }
+}
 
 // kSparse = false compiles the DENSE mode only (no predicate, no vote, V always fetched);
 // kDebug adds the optional skip_mask_out / margin_out parity outputs.
@@ -174,7 +174,6 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     constexpr int BR = 128 / G;
     constexpr int kSubD = D / 64;
     constexpr uint32_t kIdescQK = umma_idesc_bf16(128, BC, 0);   // S = Q K^T: A, B both K-major
-    constexpr uint32_t kIdescQKh = umma_idesc_bf16(128, BC / 2, 0);   // one half of the keys of a tile
     constexpr uint32_t kIdescPV = umma_idesc_bf16(128, D, 1);    // O += P V: B = V is MN-major (d contiguous)
 
     extern __shared__ uint8_t smem_raw[];
@@ -191,20 +190,13 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     auto k_empty = [&](int s) { return bar0 + 8u * (2 + NK + s); };
     auto v_full = [&](int s) { return bar0 + 8u * (2 + 2 * NK + s); };
     auto v_empty = [&](int s) { return bar0 + 8u * (2 + 2 * NK + NV + s); };
-    constexpr int kB = 2 + 2 * NK + 2 * NV;
-    auto s_full = [&](int x) { return bar0 + 8u * (kB + x); };        // S_X(j) complete in TMEM
-    auto p_half = [&](int x) { return bar0 + 8u * (kB + 2 + x); };    // first half of P_X written (kept tiles only)
-    auto p_ready = [&](int x) { return bar0 + 8u * (kB + 4 + x); };   // all of P_X written (kept tiles only)
-    auto o_full = [&](int x) { return bar0 + 8u * (kB + 6 + x); };    // last P V of slot X complete
-    auto s_read = [&](int x) { return bar0 + 8u * (kB + 8 + x); };    // the 4 warps of slot X hold S_X(j) in registers
-    // the 4 warps of slot X have voted on tile j.  A ring of 4 barriers (and 4 vote words per warp), indexed by
-    // j & 3: the votes are read by the slot's MMA warp, by the V warp and by the slot's own all-skip warps.  Slot x
-    // can only vote on tile j + 3 after its MMA warp has finished tile j + 1, which waits for v_full of tile j + 1,
-    // which the V warp completes only after it has read every vote on tile j: a ring of 4 can never be lapped.
-    auto dec = [&](int x, int q) { return bar0 + 8u * (kB + 10 + 4 * x + q); };
+    // per-slot block (see SmemLayout).  dec / votes are rings of 4 indexed by j & 3: the votes are read by the slot's
+    // MMA warp, by the V warp and by the slot's own all-skip warps.  Slot x can only vote on tile j + 3 after its MMA
+    // warp has finished tile j + 1, which waits for v_full of tile j + 1, which the V warp completes only after it has
+    // read every vote on tile j: a ring of 4 can never be lapped.
+    auto slot = [&](int x) { return sbase + L::kSlotOff + static_cast<uint32_t>(x) * L::kSlotStride; };
+    const uint32_t prog0 = sbase + L::kMiscOff + 8;                  // prog[2]: tiles finished by each issuer (gate)
     volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + L::kMiscOff);
-    volatile int* votes = reinterpret_cast<volatile int*>(smem + L::kVotesOff);                  // [2][4][4]
-    volatile float* wmax = reinterpret_cast<volatile float*>(smem + L::kVotesOff + 128);         // [2][4][4]
 
     const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);   // warp-uniform: role and slot indices live in uniform registers
     const int lane = threadIdx.x & 31;
@@ -220,20 +212,22 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         prefetch_tmap(&tm_k);
         prefetch_tmap(&tm_v);
         for (int x = 0; x < 2; ++x) {
+            const uint32_t sb = slot(x);
             mbar_init(q_full(x), 1);
-            mbar_init(s_full(x), 1);
-            mbar_init(p_half(x), 128);
-            mbar_init(p_ready(x), 128);
-            mbar_init(o_full(x), 1);
-            for (int q = 0; q < 4; ++q) mbar_init(dec(x, q), 4);
-            mbar_init(s_read(x), 4);
+            mbar_init(sb + L::kSFull, 1);
+            mbar_init(sb + L::kPHalf, 128);
+            mbar_init(sb + L::kPReady, 128);
+            mbar_init(sb + L::kOFull, 1);
+            mbar_init(sb + L::kSRead, 4);
+            for (int q = 0; q < 4; ++q) mbar_init(sb + L::kDec + 8 * q, 4);
+            for (int i = 0; i < 16; ++i) st_shared_u32(sb + L::kVotes + 4 * i, 0xffffffffu);
         }
         // a K stage is released by one softmax lane per active slot (when S_x of that tile is complete),
         // a V slot by the MMA warp of every active slot (after its P V, or at once if it skipped the tile)
         for (int s = 0; s < NK; ++s) { mbar_init(k_full(s), 1); mbar_init(k_empty(s), nX); }
         for (int s = 0; s < NV; ++s) { mbar_init(v_full(s), 1); mbar_init(v_empty(s), nX); }
-        for (int i = 0; i < 32; ++i) votes[i] = -1;
-        for (int i = 0; i < 12; ++i) reinterpret_cast<volatile int*>(smem + L::kLockOff)[i] = 0;  // in_exp, prog
+        st_shared_u32(prog0, 0u);
+        st_shared_u32(prog0 + 4, 0u);
         fence_mbar_init();
     }
     if (warp == kMmaWarp0) {
@@ -281,17 +275,17 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 if (j >= NV) mbar_wait(v_empty(j % NV), static_cast<uint32_t>((j / NV) - 1) & 1u);
             };
             auto load_v = [&](int j) {
-                const int slot = j % NV;
+                const int vs = j % NV;
                 wait_slot_free(j);
                 if (elect_one_sync()) {
-                    mbar_arrive_expect_tx(v_full(slot), L::kKVStageBytes);
+                    mbar_arrive_expect_tx(v_full(vs), L::kKVStageBytes);
                     for (int h = 0; h < kSubD; ++h)
-                        tma_load_3d(v_smem + slot * L::kKVStageBytes + h * L::kSubKVBytes, &tm_v, h * 64, j * BC, bh,
-                                    v_full(slot));
+                        tma_load_3d(v_smem + vs * L::kKVStageBytes + h * L::kSubKVBytes, &tm_v, h * 64, j * BC, bh,
+                                    v_full(vs));
                 }
                 __syncwarp();
             };
-            if (!kSparse || (DSA_EXP & 4)) {
+            if (!kSparse) {
                 for (int j = 0; j < T_c; ++j) load_v(j);
             } else {
                 // Sparse modes: V_j is needed iff some slot keeps tile j.  This warp reads the votes of both slots
@@ -307,8 +301,8 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     bool have_next = false;
                     bool keep = false;
                     for (int x = 0; x < nX; ++x) {           // act on the first keep vote, do not wait for both slots
-                        mbar_wait(dec(x, q), (j >> 2) & 1);
-                        const int4 vt = lds128_volatile(sbase + L::kVotesOff + (x * 4 + q) * 16);
+                        mbar_wait(slot(x) + L::kDec + 8 * q, (j >> 2) & 1);
+                        const int4 vt = lds128_volatile(slot(x) + L::kVotes + 16 * q);
                         keep |= (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
                         if (keep) {
                             if (!have) { load_v(j); have = true; }
@@ -327,22 +321,18 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             // ========================================================== MMA issuer(s) (a2, a6)
             // kIssuers == 2: warp 9 drives slot 0 and warp 11 slot 1.  kIssuers == 1: warp 9 drives both slots in turn
             // (warp 11 idles), which forces the two slots into anti-phase -- the best schedule when every tile is kept.
-            constexpr int kIssuers = kSparse ? DSA_ISSUERS_SPARSE : DSA_ISSUERS_DENSE;
-            constexpr bool kGate = kIssuers == 2 && DSA_GATE;
-            constexpr bool kEarlyB = DSA_EARLY_B;
+            constexpr int kIssuers = kSparse ? 2 : 1;
+            constexpr bool kGate = kIssuers == 2;
             const int x_lo = (kIssuers == 2 && warp == kMmaWarp1) ? 1 : 0;
             const int x_hi = (kIssuers == 2) ? x_lo + 1 : nX;        // this warp drives slots [x_lo, x_hi)
             if ((kIssuers == 2 || warp == kMmaWarp0) && x_lo < nX) {
-            // S_x = Q_x K^T for the keys of half h of the tile (h = 0: keys [0, BC/2) -> columns [0, BC/2) of S_x,
-            // h = 1: the other half; h = 2: the whole tile in one N = BC instruction per k step)
-            auto issue_qk = [&](int x, uint32_t kaddr, int h = 2) {
+            auto issue_qk = [&](int x, uint32_t kaddr) {             // S_x = Q_x K^T, one N = BC instruction per k step
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
                     const uint32_t off = (kk >> 2) * L::kSubQBytes + (kk & 3) * 32;
-                    const uint32_t koff = (kk >> 2) * L::kSubKVBytes + (kk & 3) * 32 + (h == 1 ? (BC / 2) * 128 : 0);
-                    umma_ss(tmem_base + x * BC + (h == 1 ? BC / 2 : 0),
-                            umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
-                            umma_smem_desc_sw128(kaddr + koff, 16, 1024), h == 2 ? kIdescQK : kIdescQKh, kk > 0);
+                    const uint32_t koff = (kk >> 2) * L::kSubKVBytes + (kk & 3) * 32;
+                    umma_ss(tmem_base + x * BC, umma_smem_desc_sw128(q_smem + x * L::kQSlotBytes + off, 16, 1024),
+                            umma_smem_desc_sw128(kaddr + koff, 16, 1024), kIdescQK, kk > 0);
                 }
             };
             // half 0 / 1: keys [0, BC/2) / [BC/2, BC); mask (SUB > 1): bit s set = decision sub-tile s was kept
@@ -363,7 +353,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             if (elect_one_sync()) {
                 for (int x = x_lo; x < x_hi; ++x) {
                     issue_qk(x, k_smem);
-                    umma_commit(s_full(x));
+                    umma_commit(slot(x) + L::kSFull);
                 }
             }
             __syncwarp();
@@ -385,34 +375,24 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 #pragma unroll
                 for (int x = 0; x < 2; ++x) {
                     if (x < x_lo || x >= x_hi) continue;
-                    // As soon as the softmax warps hold S_x(j) in registers (barrier s_read), the second half of
-                    // S_x(j+1) is issued: its columns are not needed for P_x(j), which occupies the first BC/2 columns
-                    // only, so this half of the next Q K^T is off the chain P ready -> P V -> Q K^T -> S ready.
-                    // In a run of skipped tiles the first half follows at once (speculation, see above).
+                    const uint32_t sb = slot(x);
                     const bool spec = kSparse && prev_skip[x] && has_next;
-                    if (has_next && (kEarlyB || spec)) {
-                        mbar_wait(s_read(x), j & 1);
-                        TRACE(12)
+                    if (spec) {
+                        mbar_wait(sb + L::kSRead, j & 1);
                         tc_fence_after();
                         if (elect_one_sync()) {
-                            if (kEarlyB) issue_qk(x, kaddr, 1);
-                            if (spec) {
-                                issue_qk(x, kaddr, kEarlyB ? 0 : 2);
-                                umma_commit(s_full(x));
-                            }
+                            issue_qk(x, kaddr);
+                            umma_commit(sb + L::kSFull);
                         }
                         __syncwarp();
-                        TRACE(13)
                     }
                     bool keep = true;
-                    if (kSparse && !(DSA_EXP & 2)) {
-                        TRACE(0)
+                    if (kSparse) {
                         const int q = j & 3;
-                        mbar_wait(dec(x, q), (j >> 2) & 1);  // all 4 warps of slot x have voted on tile j
-                        tc_fence_after();                    // (their votes follow their tcgen05.ld of S_x(j))
-                        TRACE(1)
+                        mbar_wait(sb + L::kDec + 8 * q, (j >> 2) & 1);   // all 4 warps of slot x have voted on tile j
+                        tc_fence_after();                                // (their votes follow their tcgen05.ld of S_x(j))
                         const int tag_keep = (j << 2) | 2;
-                        const int4 vt = lds128_volatile(sbase + L::kVotesOff + (x * 4 + q) * 16);
+                        const int4 vt = lds128_volatile(sb + L::kVotes + 16 * q);
                         keep = (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
                         prev_skip[x] = !keep;
                     }
@@ -422,42 +402,40 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         // anti-phase (softmax of one under the MMAs of the other); a slot that skips never waits, and
                         // the speculative issues above run side by side.  Scheduling only.
                         const int need = (x == 0) ? j : j + 1;
-                        while (static_cast<int>(ld_shared_u32(sbase + L::kProgOff + 4 * (1 - x))) < need) { }
+                        while (static_cast<int>(ld_shared_u32(prog0 + 4 * (1 - x))) < need) { }
                     }
                     if (keep) {
-                        mbar_wait(p_half(x), ppar[x]);
+                        mbar_wait(sb + L::kPHalf, ppar[x]);
                         mbar_wait(v_full(vslot), vph);       // V_j has landed (sparse modes: fetched by the V warp
                         tc_fence_after();                    // once some slot voted to keep tile j, or prefetched)
                         uint32_t pvmask = 0xffu;
-                        if (SUB > 1) pvmask = ld_shared_u32(sbase + L::kPvMaskOff + (x * 4 + (j & 3)) * 4);
+                        if (SUB > 1) pvmask = ld_shared_u32(sb + L::kPvMask + 4 * (j & 3));
                         if (elect_one_sync()) issue_pv(x, vaddr, j > 0, 0, pvmask);
                         __syncwarp();
-                        mbar_wait(p_ready(x), ppar[x]);
+                        mbar_wait(sb + L::kPReady, ppar[x]);
                         tc_fence_after();
                         ppar[x] ^= 1u;
                         uint32_t pvmask2 = 0xffu;            // the mask is complete once all of P_x has been handed over
-                        if (SUB > 1) pvmask2 = ld_shared_u32(sbase + L::kPvMaskOff + (x * 4 + (j & 3)) * 4);
-                        TRACE(2)
+                        if (SUB > 1) pvmask2 = ld_shared_u32(sb + L::kPvMask + 4 * (j & 3));
                         if (elect_one_sync()) {
                             issue_pv(x, vaddr, true, 1, pvmask2);
                             umma_commit(v_empty(vslot));     // this slot's P_x V_j has read V_j
                             if (has_next) {
-                                issue_qk(x, kaddr, kEarlyB ? 0 : 2);   // (again, if a speculative one was overwritten by P_x)
-                                umma_commit(s_full(x));
+                                issue_qk(x, kaddr);          // (again, if a speculative one was overwritten by P_x)
+                                umma_commit(sb + L::kSFull);
                             } else {
-                                umma_commit(o_full(x));
+                                umma_commit(sb + L::kOFull);
                             }
                         }
                         __syncwarp();
                     } else {
-                        TRACE(2)
                         if (!spec) {
                             if (elect_one_sync()) {
                                 if (has_next) {
-                                    issue_qk(x, kaddr, kEarlyB ? 0 : 2);
-                                    umma_commit(s_full(x));
+                                    issue_qk(x, kaddr);
+                                    umma_commit(sb + L::kSFull);
                                 } else {
-                                    umma_commit(o_full(x));
+                                    umma_commit(sb + L::kOFull);
                                 }
                             }
                             __syncwarp();
@@ -467,8 +445,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         if (lane == 0) mbar_arrive(v_empty(vslot));
                         __syncwarp();
                     }
-                    if (kGate && nX == 2 && lane == 0) st_shared_u32(sbase + L::kProgOff + 4 * x, static_cast<uint32_t>(j + 1));
-                    TRACE(3)
+                    if (kGate && nX == 2 && lane == 0) st_shared_u32(prog0 + 4 * x, static_cast<uint32_t>(j + 1));
                 }
                 if (has_next && ++kstage == NK) { kstage = 0; kphase ^= 1u; }
             }
@@ -496,47 +473,55 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         const float scale_log2 = a.scale_log2;
         const float lambda_log2 = a.lambda_log2;
         const bool want_margin = kDebug && a.margin != nullptr;
+        // This slot's barrier / vote block, this warp's vote word and the K-stage release ring: opaque to the compiler,
+        // so that it keeps them in registers instead of re-deriving them from the shared-memory window base every tile
+        // (which put ~60 instructions between the row max and the first exponential of a retained tile).
+        uint32_t sb = slot(x);
+        uint32_t vote_w = sb + L::kVotes + 4 * w;
+        asm volatile("" : "+r"(sb), "+r"(vote_w));
+        uint32_t kst = 0;                                    // K stage of tile j (w == 0 releases it)
 
-        constexpr bool kUseExpLock = DSA_EXP_LOCK == 2 || (DSA_EXP_LOCK == 1 && (kSparse ? DSA_ISSUERS_SPARSE : DSA_ISSUERS_DENSE) == 2);
-        // MASS mode: -lse_r in log2 units (+... rows beyond N contribute nothing)
+        // MASS mode: -lse_r in log2 units (rows beyond N contribute nothing)
         float neg_lse2 = -INFINITY;
         if (kMass && row_valid) neg_lse2 = -a.lse_in[static_cast<size_t>(bh) * a.N + grow] * kLog2e;
         float m_used = -INFINITY;   // stabiliser actually subtracted (log2 domain, may lag the true max)
+        float m_gate = -INFINITY;   // m_used + kRescaleThreshold
         float m_true = -INFINITY;   // running max over retained tiles (log2 domain) -- FIXED mode reference
         float l = 0.f;              // sum over retained tiles of 2^(s - m_used)
         float lse2 = -INFINITY;     // m_used + log2(l): LSE over retained tiles, log2 domain (Eq. 6) -- DYNAMIC reference
-        int n_exec = 0, n_skip = 0;
+        // Skip threshold of this row, log2 domain: the row votes "skip" iff mhat < thr, thr = reference + lambda
+        // (Eq. 5: t = mhat - reference < lambda).  -inf before the first retained tile (tile 0 is kept: t = +inf);
+        // rows beyond N carry lambda = +inf and never hold a tile (R9).  MASK mode: +inf / -inf from the bitmap.
+        const float lam_row = row_valid ? lambda_log2 : INFINITY;
+        float thr = -INFINITY;
+        int n_skip = 0;             // decision tiles this (leader) thread saw skipped; executed = all - skipped
         uint32_t sfpar = 0;         // parity of s_full(x): one phase per S_x issued (two for a tile re-issued after a
                                     // mis-speculated skip)
         bool prev_skip = false;     // did this slot skip tile j-1?
-        PROF_DECL(8)
 
         for (int j = 0; j < T_c; ++j) {
-            PROF_TICK(0)
-            if (w == 0) { TRACE(4) }
             // MASK mode: this tile's byte is fetched before the wait for S_x(j), which hides the global-memory latency
-            bool mask_skip = false;
-            if (kSparse && mode == kModeMask) mask_skip = (j > 0) && (!grp_valid || __ldg(a.mask_in + tile_row + j) != 0);
-            mbar_wait(s_full(x), sfpar);
+            if (kSparse && !kMass && SUB == 1 && mode == kModeMask) {
+                const bool mask_skip = (j > 0) && (!grp_valid || __ldg(a.mask_in + tile_row + j) != 0);
+                thr = mask_skip ? INFINITY : -INFINITY;
+            }
+            mbar_wait(sb + L::kSFull, sfpar);
             sfpar ^= 1u;
             tc_fence_after();
             // S_x(j) is complete, so this slot's Q K^T has read K_j for the last time (a mis-speculated S_x(j) was
             // consumed, and issued again, during tile j-1): release this slot's hold on the K stage
-            if (w == 0 && lane == 0) mbar_arrive(k_empty(j % NK));
-            if (w == 0) { TRACE(5) }
-            PROF_TICK(1)
+            if (w == 0 && lane == 0) mbar_arrive(k_empty(0) + 8 * kst);
+            if (++kst == NK) kst = 0;
             uint32_t su[BC / 32][32];                         // this thread's row of S_ij (fp32 bits)
 #pragma unroll
             for (int c = 0; c < BC / 32; ++c) tmem_ld_x32(tS + c * 32, su[c]);
             tmem_wait_ld();
             // inside a run of skipped tiles the MMA warp issues S_x(j+1) as soon as S_x(j) has left TMEM
             const bool spec = kSparse && prev_skip && (j + 1) < T_c;
-            if (kSparse || DSA_EARLY_B) {                    // S_x(j) has left TMEM
+            if (kSparse) {                                   // S_x(j) has left TMEM
                 tc_fence_before();
-                if (lane == 0) mbar_arrive(s_read(x));
+                if (lane == 0) mbar_arrive(sb + L::kSRead);
             }
-            if (w == 0) { TRACE(6) }
-            PROF_TICK(2)
 #define S_AT(c) __uint_as_float(su[(c) >> 5][(c) & 31])
             const int valid_cols = a.N - j * BC;             // ragged last K tile: columns beyond N are -inf
             if (valid_cols < BC) {
@@ -545,23 +530,56 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     if (c >= valid_cols) su[c >> 5][c & 31] = 0xff800000u;
             }
             if constexpr (kMass) {
-                // Block mass of the dense attention probabilities: sum over the rows of this warp and the columns of the
-                // tile of e^(S_rc - lse_r) (the quantity Top-K / Top-P block selection ranks).  No P, no
-                // P V: the tile is voted "skipped", so the issuer streams Q K^T only.
-                float acc0 = 0.f, acc1 = 0.f;
+                // Block mass of the dense attention probabilities: sum over the rows of the Q tile and the columns of the
+                // K tile of p = e^(S_rc - lse_r) (the quantity Top-K / Top-P block selection ranks), and
+                // optionally of p^2 (the per-tile term of Eq. 3's variance bound).  No P, no P V: the tile is
+                // voted "skipped", so the issuer streams Q K^T only.  Packed FFMA2 / FADD2 chains as in the forward
+                // kernel; one shared-memory exchange and one atomicAdd per (decision tile, K tile).
+                const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
+                const uint64_t nl2 = pack_f32x2(neg_lse2, neg_lse2);
+                const bool want_sq = a.sqmass_out != nullptr;
+                uint64_t acc2 = pack_f32x2(0.f, 0.f), sq2 = pack_f32x2(0.f, 0.f);
 #pragma unroll
                 for (int c = 0; c < BC; c += 2) {
-                    acc0 += fast_exp2(fmaf(S_AT(c), scale_log2, neg_lse2));
-                    acc1 += fast_exp2(fmaf(S_AT(c + 1), scale_log2, neg_lse2));
+                    float x0, x1;
+                    unpack_f32x2(fma_f32x2(pack_f32x2(S_AT(c), S_AT(c + 1)), scale2, nl2), x0, x1);
+                    const uint64_t p2 = pack_f32x2(fast_exp2(x0), fast_exp2(x1));
+                    acc2 = add_f32x2(acc2, p2);
+                    if (want_sq) sq2 = fma_f32x2(p2, p2, sq2);
                 }
-                float acc = row_valid ? acc0 + acc1 : 0.f;
+                float a0, a1, q0, q1;
+                unpack_f32x2(acc2, a0, a1);
+                unpack_f32x2(sq2, q0, q1);
+                float acc = row_valid ? a0 + a1 : 0.f;
+                float sq = row_valid ? q0 + q1 : 0.f;
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-                if (lane == 0 && grp_valid) atomicAdd(a.mass_out + tile_row + j, acc);
+                for (int o = 16; o > 0; o >>= 1) {
+                    acc += __shfl_xor_sync(0xffffffffu, acc, o);
+                    if (want_sq) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+                }
+                // the 4 (G = 1) or 2 (G = 2) warps of a decision tile combine through the wmax ring (one barrier), so
+                // that one thread issues one atomic per tile
+                const uint32_t wm = sb + L::kWmax + 16 * (j & 3);
+                const uint32_t wq = sb + L::kPre + 16 * (j & 3);
+                if (lane == 0) {
+                    st_shared_u32(wm + 4 * w, __float_as_uint(acc));
+                    if (want_sq) st_shared_u32(wq + 4 * w, __float_as_uint(sq));
+                }
+                named_bar_sync(1 + x, 128);
+                if (lane == 0 && (w % (4 / G)) == 0 && grp_valid) {
+                    float tot = 0.f, tsq = 0.f;
+#pragma unroll
+                    for (int i = 0; i < 4 / G; ++i) {
+                        tot += __uint_as_float(ld_shared_u32(wm + 4 * (w + i)));
+                        if (want_sq) tsq += __uint_as_float(ld_shared_u32(wq + 4 * (w + i)));
+                    }
+                    atomicAdd(a.mass_out + tile_row + j, tot);
+                    if (want_sq) atomicAdd(a.sqmass_out + tile_row + j, tsq);
+                }
                 tc_fence_before();
                 if (lane == 0) {
-                    votes[(x * 4 + (j & 3)) * 4 + w] = (j << 2) | 1;
-                    mbar_arrive(dec(x, j & 3));
+                    st_shared_u32(vote_w + 16 * (j & 3), static_cast<uint32_t>((j << 2) | 1));
+                    mbar_arrive(sb + L::kDec + 8 * (j & 3));
                 }
                 __syncwarp();
                 prev_skip = true;
@@ -578,8 +596,6 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             mx0 = fmax3(mx0, S_AT(BC - 4), S_AT(BC - 3));
             mx1 = fmax3(mx1, S_AT(BC - 2), S_AT(BC - 1));
             const float mhat2 = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;   // tile-local row max (a3)
-            if (w == 0) { TRACE(7) }
-            PROF_TICK(3)
 
             if constexpr (SUB > 1) {
                 // ============ decision tiles of BC / SUB keys: SUB decisions per MMA tile, in key order
@@ -636,20 +652,21 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     // LSE' <= log2(2^LSE + BC * 2^mhat) (DYNAMIC), m' <= max(m, mhat) (FIXED).  A row whose t stays
                     // >= lambda even against that bound keeps its sub-tile for certain, with no second vote (bits
                     // SUB..2 SUB-1).  1e-3 covers the rounding of the approximate ex2 / lg2 in the running statistics.
-                    const float grow = ((mode == kModeDynamic) ? fast_log2(1.f + static_cast<float>(BC) * fast_exp2(mhat2 - ref0))
-                                                               : fmaxf(0.f, mhat2 - ref0)) + 1e-3f;
+                    const float grow_ref = ((mode == kModeDynamic) ? fast_log2(1.f + static_cast<float>(BC) * fast_exp2(mhat2 - ref0))
+                                                                   : fmaxf(0.f, mhat2 - ref0)) + 1e-3f;
                     uint32_t wc = 0u;
 #pragma unroll
                     for (int s = 0; s < SUB; ++s) {
                         const bool rs = (j * SUB + s > 0) && (!row_valid || (msub[s] - ref0 < lambda_log2));
                         if (!__all_sync(0xffffffffu, rs)) wc |= 1u << s;
-                        const bool sure = row_valid && (msub[s] - ref0 - grow >= lambda_log2);
+                        const bool sure = row_valid && (msub[s] - ref0 - grow_ref >= lambda_log2);
                         if (__any_sync(0xffffffffu, sure)) wc |= 1u << (SUB + s);
                     }
-                    volatile uint32_t* pre = reinterpret_cast<volatile uint32_t*>(smem + L::kPreOff) + (x * 4 + (j & 1)) * 4;
-                    if (lane == 0) pre[w] = wc;
+                    const uint32_t pre = sb + L::kPre + 16 * (j & 1);
+                    if (lane == 0) st_shared_u32(pre + 4 * w, wc);
                     named_bar_sync(1 + x, 128);
-                    cand = pre[0] | pre[1] | pre[2] | pre[3];
+                    const int4 p4 = lds128_volatile(pre);
+                    cand = static_cast<uint32_t>(p4.x | p4.y | p4.z | p4.w);
                 }
                 uint32_t kept = 0u;                          // bit s: decision sub-tile s retained
                 bool half_sent = false;
@@ -682,16 +699,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
 #pragma unroll
                         for (int c = s * (W / 32); c < (s + 1) * (W / 32); ++c) {
                             uint32_t pk[16];
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) {
-                                float x0, x1;
-                                unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(su[c][2 * i]), __uint_as_float(su[c][2 * i + 1])),
-                                                       scale2, negm2), x0, x1);
-                                const float p0 = fast_exp2(x0);
-                                const float p1 = fast_exp2(x1);
-                                rs2 = add_f32x2(rs2, pack_f32x2(p0, p1));
-                                pk[i] = pack_bf16x2(p0, p1);
-                            }
+                            exp_chunk(su[c], scale2, negm2, rs2, pk);
                             tmem_st_x16(tS + c * 16, pk);
                         }
                     };
@@ -704,14 +712,17 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         // A sub-tile that follows a retained one is exponentiated BEFORE its vote is settled: the
                         // all-rows vote (shared-memory words + one barrier) then completes in the shadow of the ex2
                         // work instead of holding it up.  If the vote says skip, the P columns just written are never
-                        // read (mask bit clear) and the row sum is dropped.
+                        // read (mask bit clear) and the row sum is dropped.  Every sub-tile has its own group of vote
+                        // words: a sub-tile in between may be settled without a barrier, so a fast warp can be a whole
+                        // sub-tile ahead of a slow one that is still reading the previous group.
                         exp_sub();
                         did_exp = true;
                         const bool wv = __all_sync(0xffffffffu, row_skip);
-                        volatile uint32_t* sv = reinterpret_cast<volatile uint32_t*>(smem + L::kPreOff) + (x * 4 + 2 + (s & 1)) * 4;
-                        if (lane == 0) sv[w] = wv ? 1u : 0u;
+                        const uint32_t sv = sb + L::kPre + 16 * (1 + s);
+                        if (lane == 0) st_shared_u32(sv + 4 * w, wv ? 1u : 0u);
                         named_bar_sync(1 + x, 128);
-                        skip_s = (sv[0] & sv[1] & sv[2] & sv[3]) != 0u;   // all 128 rows of the Q tile (R1)
+                        const int4 v4 = lds128_volatile(sv);
+                        skip_s = (v4.x & v4.y & v4.z & v4.w) != 0;   // all 128 rows of the Q tile (R1)
                     } else {
                         skip_s = named_bar_red_and(1 + x, 128, row_skip);
                     }
@@ -721,10 +732,12 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             float tm = row_valid ? t2 : -INFINITY;
 #pragma unroll
                             for (int o = 16; o > 0; o >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, o));
-                            if (lane == 0) wmax[(x * 4 + q) * 4 + w] = tm;
+                            const uint32_t wm = sb + L::kWmax + 16 * q;
+                            if (lane == 0) st_shared_u32(wm + 4 * w, __float_as_uint(tm));
                             named_bar_sync(1 + x, 128);
-                            gm = fmaxf(fmaxf(wmax[(x * 4 + q) * 4 + 0], wmax[(x * 4 + q) * 4 + 1]),
-                                       fmaxf(wmax[(x * 4 + q) * 4 + 2], wmax[(x * 4 + q) * 4 + 3]));
+                            const int4 m4 = lds128_volatile(wm);
+                            gm = fmaxf(fmaxf(__int_as_float(m4.x), __int_as_float(m4.y)),
+                                       fmaxf(__int_as_float(m4.z), __int_as_float(m4.w)));
                             gm = (jj == 0) ? INFINITY : (gm - lambda_log2) * kLn2;
                             named_bar_sync(1 + x, 128);
                         }
@@ -734,20 +747,19 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         }
                     }
                     if (skip_s) {
-                        if (grp_leader && grp_valid) ++n_skip;
+                        ++n_skip;
                         continue;                            // a7: this decision tile leaves m, l, O untouched
                     }
-                    if (grp_leader && grp_valid) ++n_exec;
                     if (kept == 0u) {
                         // first retained sub-tile: the MMA tile is kept -- tell the issuer and the V warp now
                         tc_fence_before();
                         if (lane == 0) {
-                            votes[(x * 4 + q) * 4 + w] = (j << 2) | 2;
-                            mbar_arrive(dec(x, q));
+                            st_shared_u32(vote_w + 16 * q, static_cast<uint32_t>((j << 2) | 2));
+                            mbar_arrive(sb + L::kDec + 8 * q);
                         }
                         __syncwarp();
                         if (spec) {                          // a speculative S_x(j+1) is in flight over these columns
-                            mbar_wait(s_full(x), sfpar);
+                            mbar_wait(sb + L::kSFull, sfpar);
                             sfpar ^= 1u;
                             tc_fence_after();
                         }
@@ -760,10 +772,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     if (s == SUB / 2 - 1) {
                         // the first half of the keys is done and something in it was retained: hand it over now, so
                         // that its P V steps run while the second half is decided and exponentiated
-                        if (w == 0 && lane == 0) st_shared_u32(sbase + L::kPvMaskOff + (x * 4 + q) * 4, kept);
+                        if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
                         tmem_wait_st();
                         tc_fence_before();
-                        mbar_arrive(p_half(x));
+                        mbar_arrive(sb + L::kPHalf);
                         half_sent = true;
                     }
                 }
@@ -771,17 +783,17 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 if (kept == 0u) {                            // every sub-tile skipped: the MMA tile is skipped
                     tc_fence_before();
                     if (lane == 0) {
-                        votes[(x * 4 + q) * 4 + w] = (j << 2) | 1;
-                        mbar_arrive(dec(x, q));
+                        st_shared_u32(vote_w + 16 * q, static_cast<uint32_t>((j << 2) | 1));
+                        mbar_arrive(sb + L::kDec + 8 * q);
                     }
                     __syncwarp();
                     continue;
                 }
-                if (w == 0 && lane == 0) st_shared_u32(sbase + L::kPvMaskOff + (x * 4 + q) * 4, kept);
+                if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
                 tmem_wait_st();
                 tc_fence_before();
-                if (!half_sent) mbar_arrive(p_half(x));      // (release: the mask above is visible to the issuer)
-                mbar_arrive(p_ready(x));
+                if (!half_sent) mbar_arrive(sb + L::kPHalf); // (release: the mask above is visible to the issuer)
+                mbar_arrive(sb + L::kPReady);
                 fold();                                      // statistics for the next tile, behind the hand-over
                 continue;
             }
@@ -789,84 +801,76 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             bool skip_grp = false, keep_any = true;
             float grp_margin = INFINITY;
             if (kSparse) {
-                // votes[x][j & 3][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
+                // votes[j & 3][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
                 // The MMA warp combines the four votes itself (barrier dec, one arrival per warp), so an all-skip
                 // decision reaches the tensor pipe without the four warps first synchronising with each other.
-                const float ref = (mode == kModeFixed) ? m_true : lse2;
-                const float t2 = mhat2 - ref;                // Eq. 5 in log2 units (+inf at j = 0: tile 0 is kept)
-                bool row_skip = (j > 0) && (!row_valid || (t2 < lambda_log2));
-                if (mode == kModeMask) row_skip = mask_skip; // decisions read from the bitmap (one byte per decision tile)
+                const bool row_skip = mhat2 < thr;           // Eq. 5 against this row's threshold (false at j = 0)
                 const bool wskip = __all_sync(0xffffffffu, row_skip);
-                const int q = j & 3;
-                volatile int* vt = votes + (x * 4 + q) * 4;     // ring of 4 tiles (see dec)
+                const uint32_t q16 = static_cast<uint32_t>(j & 3) << 4;
                 tc_fence_before();                           // S_x(j) is in registers: the MMA warp may overwrite it
-                if (lane == 0 && !(DSA_EXP & 8)) {
-                    vt[w] = (j << 2) | (wskip ? 1 : 2);
-                    mbar_arrive(dec(x, q));
+                if (lane == 0) {
+                    st_shared_u32(vote_w + q16, static_cast<uint32_t>((j << 2) | (wskip ? 1 : 2)));
+                    mbar_arrive(sb + L::kDec + (q16 >> 1));
                 }
                 __syncwarp();
-                if (w == 0) { TRACE(8) }
                 if (kDebug) {
+                    const uint32_t wm = sb + L::kWmax + q16;
                     if (want_margin) {
-                        float tm = row_valid ? t2 : -INFINITY;
+                        const float ref = (mode == kModeFixed) ? m_true : lse2;
+                        float tm = row_valid ? mhat2 - ref : -INFINITY;      // t of Eq. 5 (+inf at j = 0)
 #pragma unroll
                         for (int o = 16; o > 0; o >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, o));
-                        if (lane == 0) wmax[(x * 4 + q) * 4 + w] = tm;
+                        if (lane == 0) st_shared_u32(wm + 4 * w, __float_as_uint(tm));
                     }
                     named_bar_sync(1 + x, 128);
-                    const bool s0 = (vt[0] & 3) == 1, s1 = (vt[1] & 3) == 1, s2 = (vt[2] & 3) == 1, s3 = (vt[3] & 3) == 1;
+                    const int4 v4 = lds128_volatile(sb + L::kVotes + q16);
+                    const bool s0 = (v4.x & 3) == 1, s1 = (v4.y & 3) == 1, s2 = (v4.z & 3) == 1, s3 = (v4.w & 3) == 1;
+                    const int4 m4 = lds128_volatile(wm);
+                    const float g0 = __int_as_float(m4.x), g1 = __int_as_float(m4.y), g2 = __int_as_float(m4.z),
+                                g3 = __int_as_float(m4.w);
                     if (G == 1) {
                         skip_grp = s0 && s1 && s2 && s3;
                         keep_any = !skip_grp;
-                        if (want_margin)
-                            grp_margin = fmaxf(fmaxf(wmax[(x * 4 + q) * 4 + 0], wmax[(x * 4 + q) * 4 + 1]),
-                                               fmaxf(wmax[(x * 4 + q) * 4 + 2], wmax[(x * 4 + q) * 4 + 3]));
+                        if (want_margin) grp_margin = fmaxf(fmaxf(g0, g1), fmaxf(g2, g3));
                     } else {
                         skip_grp = grp ? (s2 && s3) : (s0 && s1);
                         keep_any = !(s0 && s1 && s2 && s3);
-                        if (want_margin)
-                            grp_margin = fmaxf(wmax[(x * 4 + q) * 4 + 2 * grp], wmax[(x * 4 + q) * 4 + 2 * grp + 1]);
+                        if (want_margin) grp_margin = grp ? fmaxf(g2, g3) : fmaxf(g0, g1);
                     }
                     if (want_margin) grp_margin = (j == 0) ? INFINITY : (grp_margin - lambda_log2) * kLn2;
                     named_bar_sync(1 + x, 128);              // wmax / votes are reused by the next tile
-                } else if (!wskip) {
-                    skip_grp = false;                        // a row of this warp keeps the tile: no need to wait
-                    keep_any = true;
-                } else {
+                    if (grp_leader && grp_valid) {
+                        if (a.skip_mask) a.skip_mask[tile_row + j] = skip_grp ? 1 : 0;
+                        if (want_margin) a.margin[tile_row + j] = grp_margin;
+                    }
+                } else if (wskip) {
                     // every row of this warp is below the threshold: wait (hardware-suspended, no shared-memory
                     // polling) until all four warps have voted on tile j, then read the four votes at once
-                    mbar_wait(dec(x, q), (j >> 2) & 1);
+                    mbar_wait(sb + L::kDec + (q16 >> 1), (j >> 2) & 1);
                     const int tag_keep = (j << 2) | 2;
-                    const int4 v4 = lds128_volatile(sbase + L::kVotesOff + (x * 4 + q) * 16);
+                    const int4 v4 = lds128_volatile(sb + L::kVotes + q16);
                     const bool k0 = v4.x == tag_keep, k1 = v4.y == tag_keep, k2 = v4.z == tag_keep, k3 = v4.w == tag_keep;
                     keep_any = k0 | k1 | k2 | k3;
                     if (G == 1) skip_grp = !keep_any;
                     else skip_grp = !((w >> 1) ? (k2 | k3) : (k0 | k1));
                 }
+                // (a warp with a keeping row goes straight on: skip_grp = false, keep_any = true)
+                if (skip_grp) ++n_skip;                      // a9
+            } else if (kDebug && grp_leader && grp_valid) {  // DENSE: nothing is skipped, every margin is +inf
+                if (a.skip_mask) a.skip_mask[tile_row + j] = 0;
+                if (want_margin) a.margin[tile_row + j] = INFINITY;
             }
-            if (grp_leader && grp_valid) {                   // a9 + optional parity outputs
-                if (skip_grp) ++n_skip; else ++n_exec;
-                if (kDebug) {
-                    if (a.skip_mask) a.skip_mask[tile_row + j] = skip_grp ? 1 : 0;
-                    if (want_margin) a.margin[tile_row + j] = grp_margin;
-                }
-            }
-            if (w == 0) { TRACE(9) }
-            PROF_TICK(4)
             prev_skip = kSparse && !keep_any;
-            if (kSparse && !keep_any) {                      // a7: skipped -- m, l, O untouched
-                PROF_TICK(5)
-                continue;
-            }
+            if (kSparse && !keep_any) continue;              // a7: skipped -- m, l, O untouched
             if (spec) {
                 // tile j is kept although a speculative S_x(j+1) is being written over S_x: let that MMA finish before
                 // P_x goes into the same columns (the MMA warp issues S_x(j+1) again after P_x V_j)
-                mbar_wait(s_full(x), sfpar);
+                mbar_wait(sb + L::kSFull, sfpar);
                 sfpar ^= 1u;
                 tc_fence_after();
             }
 
-            float rs0 = 0.f, rs1 = 0.f;                      // this tile's row sum, two chains
+            uint64_t rs2 = pack_f32x2(0.f, 0.f);             // this tile's row sum, one packed pair of chains
             if (kSparse && G == 2 && skip_grp) {
                 // this half skipped but its partner half kept: contribute P = 0, statistics untouched
                 uint32_t z[16];
@@ -876,16 +880,17 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 for (int c = 0; c < BC / 32; ++c) tmem_st_x16(tS + c * 16, z);
                 tmem_wait_st();
                 tc_fence_before();
-                mbar_arrive(p_half(x));
+                mbar_arrive(sb + L::kPHalf);
             } else {
                 // ---- online softmax update (a5)
                 if (j == 0) {
                     m_used = mhat2;
+                    m_gate = mhat2 + kRescaleThreshold;
                 } else {
-                    const bool need = mhat2 > m_used + kRescaleThreshold;
+                    const bool need = mhat2 > m_gate;
                     if (__any_sync(0xffffffffu, need)) {
                         const float alpha = need ? fast_exp2(m_used - mhat2) : 1.f;
-                        if (need) m_used = mhat2;
+                        if (need) { m_used = mhat2; m_gate = mhat2 + kRescaleThreshold; }
                         l *= alpha;
 #pragma unroll
                         for (int c = 0; c < D / 32; ++c) {   // O_r *= alpha (PV of tile j-1 has completed: s_full(j))
@@ -898,89 +903,43 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         }
                     }
                 }
-                m_true = fmaxf(m_true, mhat2);
-                // Warps w of the two slots share one scheduler, hence one MUFU pipe.  Two exp phases run side by side
-                // both finish late; one after the other, the first finishes early and the second no later.  More
-                // important, with one MMA issuer per slot a free-running pair of slots settles in phase (both in
-                // softmax, then both in MMA), which idles the tensor pipe half of the time.  A warp therefore starts its
-                // exp phase only when its partner is not inside one (a flag per warp, checked then set: no atomics, a
-                // rare double entry is harmless).  That shifts the slots into anti-phase.  Scheduling only.
-                if (kUseExpLock && nX == 2) {
-                    while (ld_shared_u32(sbase + L::kLockOff + 4 * ((1 - x) * 4 + w)) != 0u) { }
-                    st_shared_u32(sbase + L::kLockOff + 4 * (x * 4 + w), 1u);
-                }
-                TRACE(16 + w)
-                const float neg_m = -m_used;
-#if DSA_F32X2
                 // x = s * scale - m for two logits per FFMA2, row sums as one packed pair per FADD2
+                const float neg_m = -m_used;
                 const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
                 const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
-                uint64_t rs2 = pack_f32x2(0.f, 0.f);
 #pragma unroll
                 for (int c = 0; c < BC / 32; ++c) {          // 32 columns -> 16 packed bf16x2 -> P columns [16c, 16c+16)
                     uint32_t pk[16];
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        float x0, x1;
-                        unpack_f32x2(fma_f32x2(pack_f32x2(__uint_as_float(su[c][2 * i]), __uint_as_float(su[c][2 * i + 1])),
-                                               scale2, negm2), x0, x1);
-                        const float p0 = fast_exp2(x0);
-                        const float p1 = fast_exp2(x1);
-                        rs2 = add_f32x2(rs2, pack_f32x2(p0, p1));
-                        pk[i] = pack_bf16x2(p0, p1);
-                    }
+                    exp_chunk(su[c], scale2, negm2, rs2, pk);
                     tmem_st_x16(tS + c * 16, pk);
                     if (c == BC / 64 - 1) {                  // first half of P_X is in TMEM: its P V MMAs may start
                         tmem_wait_st();
                         tc_fence_before();
-                        mbar_arrive(p_half(x));
-                        TRACE(20 + w)
+                        mbar_arrive(sb + L::kPHalf);
                     }
                 }
-                unpack_f32x2(rs2, rs0, rs1);
-#else
-#pragma unroll
-                for (int c = 0; c < BC / 32; ++c) {          // 32 columns -> 16 packed bf16x2 -> P columns [16c, 16c+16)
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        const float x0 = fmaf(__uint_as_float(su[c][2 * i]), scale_log2, neg_m);
-                        const float x1 = fmaf(__uint_as_float(su[c][2 * i + 1]), scale_log2, neg_m);
-                        const float p0 = fast_exp2(x0);
-                        const float p1 = fast_exp2(x1);
-                        rs0 += p0;
-                        rs1 += p1;
-                        pk[i] = pack_bf16x2(p0, p1);
-                    }
-                    tmem_st_x16(tS + c * 16, pk);
-                    if (c == BC / 64 - 1) {                  // first half of P_X is in TMEM: its P V MMAs may start
-                        tmem_wait_st();
-                        tc_fence_before();
-                        mbar_arrive(p_half(x));
-                        TRACE(20 + w)
-                    }
-                }
-#endif
-                if (kUseExpLock && nX == 2) st_shared_u32(sbase + L::kLockOff + 4 * (x * 4 + w), 0u);
             }
 #undef S_AT
-            PROF_TICK(6)
             tmem_wait_st();
             tc_fence_before();
-            mbar_arrive(p_ready(x));
-            TRACE(24 + w)
-            // the statistics are updated after P has been handed over: the tail of the row-sum chain and the log2
-            // must not sit between the last exp and the arrive (in-order issue would stall the arrive on them)
+            mbar_arrive(sb + L::kPReady);
+            // The statistics are updated after P has been handed over: the tail of the row-sum chain, the log2 and the
+            // next tile's threshold must not sit between the last exp and the arrive (in-order issue would stall the
+            // arrive on them); here they run while the tensor pipe works on P_x V_j and S_x(j+1).
             if (!(kSparse && G == 2 && skip_grp)) {
+                float rs0, rs1;
+                unpack_f32x2(rs2, rs0, rs1);
                 l += rs0 + rs1;
-                if (kSparse && mode != kModeFixed && !(DSA_EXP & 16)) lse2 = m_used + fast_log2(l);
+                if (kSparse) {
+                    m_true = fmaxf(m_true, mhat2);
+                    if (mode != kModeFixed) lse2 = m_used + fast_log2(l);
+                    if (mode != kModeMask) thr = ((mode == kModeFixed) ? m_true : lse2) + lam_row;
+                }
             }
-            PROF_TICK(7)
         }
-        PROF_FLUSH(8 + 8 * x, 8, r == 0)
 
         // ---- epilogue (a8): O / l -> bf16, lse = ln(l) + m over retained tiles
-        mbar_wait(o_full(x), 0);
+        mbar_wait(sb + L::kOFull, 0);
         tc_fence_after();
         const float inv_l = 1.f / l;
         __nv_bfloat16* orow = a.out + (static_cast<size_t>(bh) * a.N + (row_valid ? grow : 0)) * D;
@@ -1003,8 +962,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
         }
         if (a.lse && row_valid && !kMass) a.lse[static_cast<size_t>(bh) * a.N + grow] = (m_used + log2f(l)) * kLn2;
-        if (a.stats && grp_leader && grp_valid) {
-            atomicAdd(a.stats + 2 * bh + 0, static_cast<unsigned long long>(n_exec));
+        if (a.stats && grp_leader && grp_valid && !kMass) {
+            // a9: every decision tile of this Q tile is either executed or skipped (DENSE: none skipped)
+            atomicAdd(a.stats + 2 * bh + 0, static_cast<unsigned long long>(a.T_c_dec - n_skip));
             atomicAdd(a.stats + 2 * bh + 1, static_cast<unsigned long long>(n_skip));
         }
         }

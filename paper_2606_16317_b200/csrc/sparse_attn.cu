@@ -80,11 +80,8 @@ int launch(const CUtensorMap& tq, const CUtensorMap& tk, const CUtensorMap& tv, 
            cudaStream_t stream) {
     using L = dsa::SmemLayout<D, BC, NK, NV>;
     auto kernel = dsa::sparse_attn_fwd_kernel<D, BC, G, NK, NV, kSparse, kDebug, SUB>;
-    static bool configured = false;
-    if (!configured) {
-        CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L::kDynamicBytes));
-        configured = true;
-    }
+    // per device and cheap: set on every launch, so that any device / thread of the process may call the library
+    CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, L::kDynamicBytes));
     dim3 grid((args.n_mma_tiles + 1) / 2, BH, 1);
     kernel<<<grid, dsa::kNumThreads, L::kDynamicBytes, stream>>>(tq, tk, tv, args);
     CUDA_TRY(cudaGetLastError());
@@ -135,6 +132,9 @@ int validate(const void* q, const void* k, const void* v, void* out, int B, int 
         if ((tq != def_tile || tk != def_tile) && !sub_ok)
             return fail(SPARSE_ATTN_ERR_TILE, "decision tile %dx%d unsupported for D = %d in mode %d (supported: %dx%d%s)", tq, tk, D,
                         mode, def_tile, def_tile, D == 128 ? ", and 128x64 / 128x32 in the sparse modes" : "");
+        if (sub_ok && tk != def_tile && p->lambda > 0.f)
+            return fail(SPARSE_ATTN_ERR_PARAMS, "lambda = %g > 0 is unsupported with %dx%d decision tiles (the stabiliser follows the "
+                        "max of the whole 128-key MMA tile, which a positive threshold may skip)", p->lambda, tq, tk);
         r->tile_k = tk;
         if (p->softmax_scale > 0.f) r->scale = p->softmax_scale;
         r->lambda = p->lambda;
@@ -191,6 +191,7 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     if ((rc = make_tmap(enc, &tv, v, BH, N, D, mma_k))) return rc;
 
     dsa::FwdArgs a;
+    std::memset(&a, 0, sizeof a);
     a.out = static_cast<__nv_bfloat16*>(out);
     a.lse = lse;
     a.stats = reinterpret_cast<unsigned long long*>(stats_out);
@@ -205,9 +206,6 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     a.mode = mode;
     a.scale_log2 = r.scale * dsa::kLog2e;
     a.lambda_log2 = r.lambda * dsa::kLog2e;
-#ifdef DSA_PROF
-    a.prof = reinterpret_cast<unsigned long long*>(getenv("DSA_PROF_PTR") ? strtoull(getenv("DSA_PROF_PTR"), nullptr, 0) : 0ull);
-#endif
 
     if (stats_out) CUDA_TRY(cudaMemsetAsync(stats_out, 0, sizeof(int64_t) * 2 * BH, r.stream));
     const bool sparse = mode != SPARSE_ATTN_DENSE;
@@ -232,71 +230,126 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     return launch<64, 64, 2, 3, 2, true, true>(tq, tk, tv, a, BH, r.stream);
 }
 
+// Host-buffer entry: the B*H heads are independent units, so they are cut into chunks and pipelined over three
+// streams -- H2D of chunk c+1 and D2H of chunk c-1 run under the kernel of chunk c (PCIe is full duplex), and the
+// kernels of consecutive chunks alternate between two streams so that the next chunk's CTAs fill the last wave of the
+// previous one.  Device scratch comes from the stream-ordered pool (one allocation per tensor and call).
 int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse, int B, int H, int N, int D,
                          const sparse_attn_params* params, int mode, int64_t* stats_out) {
     Resolved r;
     int rc = validate(q, k, v, out, B, H, N, D, params, mode, &r);
     if (rc) return rc;
     if ((rc = check_device())) return rc;
-    const size_t n_elem = static_cast<size_t>(B) * H * N * D;
     const size_t BH = static_cast<size_t>(B) * H;
+    const size_t head_elems = static_cast<size_t>(N) * D;
     const size_t T_r = (N + r.tile_q - 1) / r.tile_q, T_c = (N + r.tile_k - 1) / r.tile_k;
+    const size_t head_tiles = T_r * T_c;
+    constexpr int kMaxChunks = 8;
+    const int n_chunks = static_cast<int>(std::min<size_t>(BH, kMaxChunks));
+    cudaStream_t st = r.stream;
+    cudaStream_t s_in = nullptr, s_out = nullptr, s_k[2] = {nullptr, nullptr};
+    cudaEvent_t ev_start = nullptr, ev_in[kMaxChunks] = {}, ev_done[kMaxChunks] = {}, ev_end[4] = {};
     void *dq = nullptr, *dk = nullptr, *dv = nullptr, *dout = nullptr;
     float *dlse = nullptr, *dmargin = nullptr;
     int64_t* dstats = nullptr;
-    uint8_t* dmask = nullptr;
-    uint8_t* dmask_in = nullptr;
-    cudaStream_t st = r.stream;
+    uint8_t *dmask = nullptr, *dmask_in = nullptr;
     auto cleanup = [&]() {
-        cudaFree(dq); cudaFree(dk); cudaFree(dv); cudaFree(dout); cudaFree(dlse); cudaFree(dstats);
-        cudaFree(dmask); cudaFree(dmargin); cudaFree(dmask_in);
+        void* bufs[] = {dq, dk, dv, dout, dlse, dstats, dmask, dmargin, dmask_in};
+        for (void* b : bufs) if (b) cudaFreeAsync(b, st);
+        cudaStreamSynchronize(st);
+        for (cudaStream_t s : {s_in, s_out, s_k[0], s_k[1]}) if (s) cudaStreamDestroy(s);
+        if (ev_start) cudaEventDestroy(ev_start);
+        for (int c = 0; c < kMaxChunks; ++c) { if (ev_in[c]) cudaEventDestroy(ev_in[c]); if (ev_done[c]) cudaEventDestroy(ev_done[c]); }
+        for (cudaEvent_t e : ev_end) if (e) cudaEventDestroy(e);
     };
 #define HOST_TRY(expr)                                                                                   \
     do {                                                                                                 \
         cudaError_t err__ = (expr);                                                                      \
         if (err__ != cudaSuccess) {                                                                      \
+            cudaDeviceSynchronize();                                                                     \
             cleanup();                                                                                   \
             return fail(SPARSE_ATTN_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(err__));        \
         }                                                                                                \
     } while (0)
-    HOST_TRY(cudaMalloc(&dq, n_elem * 2));
-    HOST_TRY(cudaMalloc(&dk, n_elem * 2));
-    HOST_TRY(cudaMalloc(&dv, n_elem * 2));
-    HOST_TRY(cudaMalloc(&dout, n_elem * 2));
-    if (lse) HOST_TRY(cudaMalloc(&dlse, BH * N * sizeof(float)));
-    if (stats_out) HOST_TRY(cudaMalloc(&dstats, BH * 2 * sizeof(int64_t)));
-    if (r.skip_mask) HOST_TRY(cudaMalloc(&dmask, BH * T_r * T_c));
-    if (r.margin) HOST_TRY(cudaMalloc(&dmargin, BH * T_r * T_c * sizeof(float)));
-    if (r.mask_in) {                                        // MASK mode: the bitmap is a host buffer here too
-        HOST_TRY(cudaMalloc(&dmask_in, BH * T_r * T_c));
-        HOST_TRY(cudaMemcpyAsync(dmask_in, r.mask_in, BH * T_r * T_c, cudaMemcpyHostToDevice, st));
+    {                            // keep freed scratch in the pool between calls instead of returning it to the driver
+        int dev = 0;
+        cudaMemPool_t pool;
+        HOST_TRY(cudaGetDevice(&dev));
+        HOST_TRY(cudaDeviceGetDefaultMemPool(&pool, dev));
+        uint64_t keep = UINT64_MAX;
+        HOST_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
     }
-    HOST_TRY(cudaMemcpyAsync(dq, q, n_elem * 2, cudaMemcpyHostToDevice, st));
-    HOST_TRY(cudaMemcpyAsync(dk, k, n_elem * 2, cudaMemcpyHostToDevice, st));
-    HOST_TRY(cudaMemcpyAsync(dv, v, n_elem * 2, cudaMemcpyHostToDevice, st));
+    HOST_TRY(cudaMallocAsync(&dq, BH * head_elems * 2, st));
+    HOST_TRY(cudaMallocAsync(&dk, BH * head_elems * 2, st));
+    HOST_TRY(cudaMallocAsync(&dv, BH * head_elems * 2, st));
+    HOST_TRY(cudaMallocAsync(&dout, BH * head_elems * 2, st));
+    if (lse) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dlse), BH * N * sizeof(float), st));
+    if (stats_out) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dstats), BH * 2 * sizeof(int64_t), st));
+    if (r.skip_mask) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dmask), BH * head_tiles, st));
+    if (r.margin) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dmargin), BH * head_tiles * sizeof(float), st));
+    if (r.mask_in) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dmask_in), BH * head_tiles, st));
+    HOST_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+    HOST_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+    HOST_TRY(cudaStreamCreateWithFlags(&s_k[0], cudaStreamNonBlocking));
+    HOST_TRY(cudaStreamCreateWithFlags(&s_k[1], cudaStreamNonBlocking));
+    HOST_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+    for (int c = 0; c < n_chunks; ++c) {
+        HOST_TRY(cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming));
+        HOST_TRY(cudaEventCreateWithFlags(&ev_done[c], cudaEventDisableTiming));
+    }
+    for (cudaEvent_t& e : ev_end) HOST_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    // the scratch allocations (and whatever the caller enqueued before) are ordered on `st`
+    HOST_TRY(cudaEventRecord(ev_start, st));
+    for (cudaStream_t s : {s_in, s_out, s_k[0], s_k[1]}) HOST_TRY(cudaStreamWaitEvent(s, ev_start, 0));
+
     sparse_attn_params dp;
     std::memset(&dp, 0, sizeof dp);
     if (params) dp = *params;
     dp.struct_size = sizeof dp;
     if (!params) dp.lambda = -INFINITY;
-    dp.skip_mask_out = dmask;
-    dp.margin_out = dmargin;
-    dp.skip_mask_in = dmask_in;
-    rc = sparse_attn_fwd(dq, dk, dv, dout, dlse, B, H, N, D, &dp, mode, dstats);
-    if (rc) { cleanup(); return rc; }
-    HOST_TRY(cudaMemcpyAsync(out, dout, n_elem * 2, cudaMemcpyDeviceToHost, st));
-    if (lse) HOST_TRY(cudaMemcpyAsync(lse, dlse, BH * N * sizeof(float), cudaMemcpyDeviceToHost, st));
-    if (stats_out) HOST_TRY(cudaMemcpyAsync(stats_out, dstats, BH * 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-    if (r.skip_mask) HOST_TRY(cudaMemcpyAsync(r.skip_mask, dmask, BH * T_r * T_c, cudaMemcpyDeviceToHost, st));
-    if (r.margin) HOST_TRY(cudaMemcpyAsync(r.margin, dmargin, BH * T_r * T_c * sizeof(float), cudaMemcpyDeviceToHost, st));
+    auto at = [](const void* p, size_t bytes) { return static_cast<const char*>(p) + bytes; };
+    auto atw = [](void* p, size_t bytes) { return static_cast<char*>(p) + bytes; };
+    for (int c = 0; c < n_chunks; ++c) {
+        const size_t h0 = BH * c / n_chunks, h1 = BH * (c + 1) / n_chunks, nh = h1 - h0;
+        const size_t eoff = h0 * head_elems * 2, ebytes = nh * head_elems * 2;
+        if (r.mask_in)
+            HOST_TRY(cudaMemcpyAsync(dmask_in + h0 * head_tiles, r.mask_in + h0 * head_tiles, nh * head_tiles, cudaMemcpyHostToDevice, s_in));
+        HOST_TRY(cudaMemcpyAsync(atw(dq, eoff), at(q, eoff), ebytes, cudaMemcpyHostToDevice, s_in));
+        HOST_TRY(cudaMemcpyAsync(atw(dk, eoff), at(k, eoff), ebytes, cudaMemcpyHostToDevice, s_in));
+        HOST_TRY(cudaMemcpyAsync(atw(dv, eoff), at(v, eoff), ebytes, cudaMemcpyHostToDevice, s_in));
+        HOST_TRY(cudaEventRecord(ev_in[c], s_in));
+        cudaStream_t sk = s_k[c & 1];
+        HOST_TRY(cudaStreamWaitEvent(sk, ev_in[c], 0));
+        dp.stream = sk;
+        dp.skip_mask_out = dmask ? dmask + h0 * head_tiles : nullptr;
+        dp.margin_out = dmargin ? dmargin + h0 * head_tiles : nullptr;
+        dp.skip_mask_in = dmask_in ? dmask_in + h0 * head_tiles : nullptr;
+        rc = sparse_attn_fwd(atw(dq, eoff), atw(dk, eoff), atw(dv, eoff), atw(dout, eoff), dlse ? dlse + h0 * N : nullptr, 1,
+                             static_cast<int>(nh), N, D, &dp, mode, dstats ? dstats + h0 * 2 : nullptr);
+        if (rc) { cudaDeviceSynchronize(); cleanup(); return rc; }
+        HOST_TRY(cudaEventRecord(ev_done[c], sk));
+        HOST_TRY(cudaStreamWaitEvent(s_out, ev_done[c], 0));
+        HOST_TRY(cudaMemcpyAsync(atw(out, eoff), at(dout, eoff), ebytes, cudaMemcpyDeviceToHost, s_out));
+        if (lse) HOST_TRY(cudaMemcpyAsync(lse + h0 * N, dlse + h0 * N, nh * N * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+        if (stats_out) HOST_TRY(cudaMemcpyAsync(stats_out + h0 * 2, dstats + h0 * 2, nh * 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, s_out));
+        if (r.skip_mask) HOST_TRY(cudaMemcpyAsync(r.skip_mask + h0 * head_tiles, dmask + h0 * head_tiles, nh * head_tiles, cudaMemcpyDeviceToHost, s_out));
+        if (r.margin)
+            HOST_TRY(cudaMemcpyAsync(r.margin + h0 * head_tiles, dmargin + h0 * head_tiles, nh * head_tiles * sizeof(float), cudaMemcpyDeviceToHost, s_out));
+    }
+    // join everything back into `st`, then wait: the call is synchronous
+    cudaStream_t joins[4] = {s_in, s_out, s_k[0], s_k[1]};
+    for (int i = 0; i < 4; ++i) {
+        HOST_TRY(cudaEventRecord(ev_end[i], joins[i]));
+        HOST_TRY(cudaStreamWaitEvent(st, ev_end[i], 0));
+    }
     HOST_TRY(cudaStreamSynchronize(st));
     cleanup();
 #undef HOST_TRY
     return 0;
 }
 
-int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float* mass_out, int B, int H, int N, int D,
-                           float softmax_scale, void* stream) {
+int sparse_attn_block_stats(const void* q, const void* k, const float* lse, float* mass_out, float* sqmass_out, int B, int H,
+                            int N, int D, float softmax_scale, void* stream) {
     g_last_error[0] = '\0';
     if (!q || !k || !lse || !mass_out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "q, k, lse and mass_out must not be NULL");
     if (B <= 0 || H <= 0 || N <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N must be positive (got %d, %d, %d)", B, H, N);
@@ -327,11 +380,38 @@ int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float
     a.lambda_log2 = -INFINITY;
     a.lse_in = lse;
     a.mass_out = mass_out;
+    a.sqmass_out = sqmass_out;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     CUDA_TRY(cudaMemsetAsync(mass_out, 0, sizeof(float) * static_cast<size_t>(BH) * a.T_r * a.T_c, st));
+    if (sqmass_out) CUDA_TRY(cudaMemsetAsync(sqmass_out, 0, sizeof(float) * static_cast<size_t>(BH) * a.T_r * a.T_c, st));
     // V is never read for P V in this mode (every tile is voted skipped); the V map aliases K for the one prefetch of tile 0
     if (D == 128) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false, 0>(tq, tk, tk, a, BH, st);
     return launch<64, 64, 2, 3, 2, true, false, 0>(tq, tk, tk, a, BH, st);
+}
+
+int sparse_attn_block_mass(const void* q, const void* k, const float* lse, float* mass_out, int B, int H, int N, int D,
+                           float softmax_scale, void* stream) {
+    return sparse_attn_block_stats(q, k, lse, mass_out, nullptr, B, H, N, D, softmax_scale, stream);
+}
+
+int sparse_attn_select_blocks_greedy(const float* mass, const float* sqmass, uint8_t* skip_mask_out, int B, int H, int N,
+                                     int tile_q, int T_c, double theta, void* stream) {
+    g_last_error[0] = '\0';
+    if (!mass || !sqmass || !skip_mask_out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "mass, sqmass and skip_mask_out must not be NULL");
+    if (B <= 0 || H <= 0 || N <= 0 || T_c <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N, T_c must be positive");
+    if (tile_q != 64 && tile_q != 128) return fail(SPARSE_ATTN_ERR_TILE, "tile_q = %d not in {64, 128}", tile_q);
+    if (static_cast<long long>(B) * H > 65535) return fail(SPARSE_ATTN_ERR_SHAPE, "B*H = %lld exceeds 65535", (long long)B * H);
+    if (T_c > dsa::kSelectMaxTc) return fail(SPARSE_ATTN_ERR_SHAPE, "T_c = %d exceeds %d", T_c, dsa::kSelectMaxTc);
+    if (!(theta >= 0.0)) return fail(SPARSE_ATTN_ERR_PARAMS, "theta = %g must be >= 0", theta);
+    int rc = check_device();
+    if (rc) return rc;
+    const int T_r = (N + tile_q - 1) / tile_q;
+    dim3 grid(T_r, B * H, 1);
+    dsa::select_blocks_greedy_kernel<<<grid, 256, sizeof(float) * 3 * T_c, static_cast<cudaStream_t>(stream)>>>(
+        mass, sqmass, skip_mask_out, T_c, N, tile_q, theta);
+    CUDA_TRY(cudaGetLastError());
+    g_reorder_launches.fetch_add(1);
+    return 0;
 }
 
 int sparse_attn_select_blocks(const float* mass, uint8_t* skip_mask_out, int B, int H, int T_r, int T_c, int kind,
