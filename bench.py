@@ -1,15 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- times the tile-skipping attention forward on synthetic Wan-2.2-shaped inputs.
 
-One "step" = one sparse_attn_fwd call (the whole hot path) over one
-batch of BASELINE.json config 1 (B=1, H=24, N=32760, D=128, 128x128 tiles) in DYNAMIC mode at the
-paper's Eq. 7 threshold (P_real = 1.5).  The same kernel's DENSE and FIXED modes are timed beside
-it, on the contract ("literal") generator and on the supplementary aligned variant.
+One "step" = one sparse_attn_fwd call (the whole hot path) over one batch of
+BASELINE.json config 3 (B=1, H=40, N=75600, D=128, 128x128 tiles: the Wan2.2-14B 720p shape the paper quotes its
+threshold for) in DYNAMIC mode at the paper's Eq. 7 threshold (P_real = 1.5 -> lambda = -5.98, the paper's "-6",
+PAPER.md:139).  The same kernel's DENSE and FIXED modes are timed beside it, on the contract generator, on the
+supplementary aligned variant and on the contract data re-ordered into bricks.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config cfgX]
+  python bench.py --report cfg2|cfg3|cfg4|masks|kurtosis     (the sweeps BASELINE.json configs[2..4] ask for; JSON)
 
-Prints ONE JSON line on rank 0.  N > 1 (under torchrun): every rank runs its own config-1 batch
-(heads are independent units: no data-path collective, weak scaling), stats are all-gathered.
+Prints ONE JSON line on rank 0.  N > 1 (under torchrun): every rank runs its own batch (heads are independent
+units: no data-path collective, weak scaling), stats are all-gathered.
 """
 from __future__ import annotations
 
@@ -17,6 +19,7 @@ import argparse
 import json
 import math
 import os
+import re
 import subprocess
 import sys
 import threading
@@ -30,14 +33,15 @@ sys.path.insert(0, ROOT)
 from workloads import CONFIGS, make_qkv  # noqa: E402
 
 METRIC = "attention ms & effective TFLOP/s vs dense mode at Wan-2.2 shapes; sparsity %; % tensor peak"
+UNIT = "TFLOP/s (dense-equivalent attention FLOP / time)"       # the same string in both arms
+DEFAULT_CONFIG = "cfg3"
 P_REAL = 1.5            # Eq. 7 "transition region" constant
 FALLBACK_TFLOPS = 1590.0
 BRICK = (4, 4, 8)       # token re-ordering brick (t, h, w): 128 tokens = one attention tile
-# dram__bytes_read.sum + dram__bytes_write.sum of one DENSE config-1 launch, ncu --set full (profiles/ncu_dense_r01.md);
-# algorithmic bytes: q + k + v + out + lse = 4 * 201.3 MB + 3.1 MB = 808 MB
-NCU_DRAM_BYTES_DENSE_CFG1 = 610.71e6 + 189.00e6
+ROUND = "r02"
 
 
+# ---------------------------------------------------------------------------------------------- peaks, names, profiles
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -47,16 +51,59 @@ def measured_peaks():
     return FALLBACK_TFLOPS, 1400.0, "fallback"
 
 
+def measured_hbm():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"])
+    return 6650.0                                           # fallback stated in B200_PROFILING.md
+
+
+def eq7_lambda(cfg, tile_k=None, p_real=P_REAL):
+    return math.log(p_real) + math.log((tile_k or cfg.tile) / cfg.N)        # Eq. 7
+
+
+def workload_name(cfg):
+    kind = "supplementary aligned variant of " if cfg.aligned else ""
+    gen = (f"per-head tau~U[1,2.5] sigma~U[1,6] a={cfg.noise_a}" if cfg.per_head
+           else f"sigma={cfg.sigma} a={cfg.noise_a} tau={cfg.tau}")
+    return (f"{kind}BASELINE.json configs[{cfg.config_id}] ({cfg.name}): B={cfg.B} H={cfg.H} N={cfg.N} (grid {cfg.grid}) "
+            f"D={cfg.D}, {cfg.tile}x{cfg.tile} tiles, generator {gen}")
+
+
+def ncu_traffic(config, mode):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, read from the tracked ncu summary of this config and
+    mode (profiles/ncu_<mode>_<config>_<round>.md, written from one `ncu --set full` capture); None if there is none."""
+    path = os.path.join(ROOT, "profiles", f"ncu_{mode}_{config}_{ROUND}.md")
+    if not os.path.exists(path):
+        return None, None
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    total = 0.0
+    with open(path) as f:
+        for line in f:
+            m = re.match(r"\|\s*dram__bytes_(read|write)\.sum\s*\|\s*([0-9.,]+)\s*\|\s*(\w+)\s*\|", line)
+            if m:
+                total += float(m.group(2).replace(",", "")) * scale[m.group(3)]
+    return (total or None), os.path.relpath(path, ROOT)
+
+
 def dense_flop(BH, N, D):
     return 4.0 * BH * N * N * D
 
 
-def executed_flop(BH, N, D, tile, stats):
+def executed_flop(BH, N, D, stats):
     """QK^T for every tile + P V for executed tiles; ragged tiles counted as full
     in the P V term (error < 1/T_c)."""
     qk = 2.0 * BH * N * N * D
     frac_exec = float(stats[..., 0].sum()) / float(stats.sum())   # executed / all decision tiles (any tile_k)
     return qk + 2.0 * BH * N * N * D * frac_exec
+
+
+def host_workers():
+    try:
+        return max(1, min(16, len(os.sched_getaffinity(0))))
+    except AttributeError:
+        return max(1, min(16, os.cpu_count() or 1))
 
 
 class ClockSampler:
@@ -108,15 +155,13 @@ class ClockSampler:
 
 # ---------------------------------------------------------------------------------------------- oracle arm
 def oracle_sample_time(cfg, seed, lam, mode, head=0, reps=1):
-    """Time the oracle, as it stands, on a bounded sample: up to 16 x (host threads) Q tiles of one head
-    (for config 1 on a 16-core box that is one full head, all 256 Q tiles)."""
+    """Time the oracle, as it stands, on a bounded sample: 4 x (host threads) evenly spaced Q tiles of one head (first
+    and ragged last included), all K tiles -- about 6 s of work per repetition at config 3 on 16 cores."""
     import oracle
     q, k, v = make_qkv(cfg, seed, heads=[head])
     cores = oracle.max_threads()
     T = -(-cfg.N // cfg.tile)
-    n_tiles = min(T, 16 * cores)
-    qt = [int(x) for x in np.linspace(0, T - 1, n_tiles).round()]
-    qt = sorted(set(qt))
+    qt = sorted(set(int(x) for x in np.linspace(0, T - 1, min(T, 4 * cores)).round()))
     times = []
     for _ in range(reps):
         t0 = time.perf_counter()
@@ -138,48 +183,103 @@ def run_reference(args, cfg, lam):
     mean_s = float(np.mean(secs))
     val = res["flop"] / mean_s / 1e12
     line = {
-        "impl": "reference", "metric": METRIC, "value": val, "unit": "TFLOP/s (dense-equivalent, effective)",
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT,
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": mean_s * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "mode": "dynamic", "lambda": lam, "step": res["sample"]},
-        "cpu_baseline": {"value": val, "unit": "TFLOP/s (dense-equivalent, effective)", "cores": res["cores"],
-                         "kind": "oracle", "sample": res["sample"]},
-        "e2e": {"value": val, "unit": "TFLOP/s (dense-equivalent, effective)", "h2d_bytes_per_step": 0,
-                "d2h_bytes_per_step": 0},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": res["cores"], "kind": "oracle", "sample": res["sample"]},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
 
 
-def workload_name(cfg):
-    return (f"BASELINE.json configs[1] ({cfg.name}): B={cfg.B} H={cfg.H} N={cfg.N} (grid {cfg.grid}) D={cfg.D}, "
-            f"{cfg.tile}x{cfg.tile} tiles, generator sigma={cfg.sigma} a={cfg.noise_a} tau={cfg.tau}")
+# ---------------------------------------------------------------------------------------------- GPU arm helpers
+class Gpu:
+    """Device buffers of one workload plus the timing / quality helpers (every value through the C ABI)."""
+
+    def __init__(self, sa, torch, cfg, qb, kb, vb, barrier=lambda: None):
+        self.sa, self.torch, self.cfg, self.barrier = sa, torch, cfg, barrier
+        self.B, self.H, self.N, self.D = qb.shape
+
+        def to_dev(bits):
+            return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).cuda().view(torch.bfloat16)
+
+        self.q, self.k, self.v = to_dev(qb), to_dev(kb), to_dev(vb)
+        self.out = torch.empty_like(self.q)
+        self.lse = torch.empty((self.B, self.H, self.N), device="cuda", dtype=torch.float32)
+        self.stats = torch.zeros((self.B, self.H, 2), device="cuda", dtype=torch.int64)
+        self.out_dense = self.lse_dense = None
+        self._rs = torch.zeros(2, device="cuda", dtype=torch.float64)
+        self.stream = torch.cuda.current_stream()
+
+    def call(self, mode, lam=-math.inf, tile_k=0, mask_in=None, skip_mask_out=None):
+        p = self.sa.make_params(lam=lam, stream=self.stream.cuda_stream, tile_q=self.cfg.tile if tile_k else 0,
+                                tile_k=tile_k, skip_mask_in=mask_in, skip_mask_out=skip_mask_out)
+        self.sa.sparse_attn_fwd(self.q, self.k, self.v, self.out, self.lse, self.B, self.H, self.N, self.D, p, mode, self.stats)
+
+    def preheat(self, seconds):
+        """Untimed DENSE calls: after the idle seconds of input generation the first timed mode would otherwise run at
+        burst clocks and the later ones under the power cap, which biases every ratio between modes by a few percent."""
+        t0 = time.perf_counter()
+        while time.perf_counter() - t0 < seconds:
+            for _ in range(4):
+                self.call(self.sa.MODE_DENSE)
+            self.torch.cuda.synchronize()
+
+    def time(self, mode, lam, steps, warmup, tile_k=0, mask_in=None, sampler=None):
+        """Returns (total_ms over `steps` calls, per-call ms list, stats [B,H,2])."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.call(mode, lam, tile_k, mask_in)
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+        self.barrier()
+        torch.cuda.synchronize()
+        if sampler is not None:
+            sampler.active.set()
+        evs[0].record(self.stream)
+        for i in range(steps):
+            self.call(mode, lam, tile_k, mask_in)
+            evs[i + 1].record(self.stream)
+        torch.cuda.synchronize()
+        if sampler is not None:
+            sampler.active.clear()
+        self.barrier()
+        per = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
+        return evs[0].elapsed_time(evs[-1]), per, self.stats.cpu().numpy().copy()
+
+    def keep_dense(self):
+        self.out_dense, self.lse_dense = self.out.clone(), self.lse.clone()
+
+    def quality(self, heads=None):
+        """Achieved recall per row = exp(lse_retained - lse_dense) and error against the dense output,
+        reduced on the device by sparse_attn_recall_stats / sparse_attn_output_error."""
+        if self.lse_dense is None:
+            return {}
+        sa, st = self.sa, self.stream.cuda_stream
+        lse, lse_d, out, out_d = self.lse, self.lse_dense, self.out, self.out_dense
+        if heads is not None:
+            h0, h1 = heads
+            lse, lse_d, out, out_d = lse[:, h0:h1], lse_d[:, h0:h1], out[:, h0:h1], out_d[:, h0:h1]
+            assert self.B == 1
+        n_rows, n_el = lse.numel(), out.numel()
+        sa.sparse_attn_recall_stats(lse, lse_d, n_rows, self._rs, st)
+        rmin, rsum = self._rs.tolist()
+        sa.sparse_attn_output_error(out, out_d, n_el, self._rs, st)
+        emax, esum = self._rs.tolist()
+        return {"recall_min": rmin, "recall_mean": rsum / n_rows, "err_vs_dense_max_abs": emax,
+                "err_vs_dense_mean_abs": esum / n_el}
 
 
-# ---------------------------------------------------------------------------------------------- GPU arm
-def time_mode(sa, torch, bufs, cfg, mode, lam, steps, warmup, barrier, sampler=None, tile_k=0, mask_in=None):
-    """Returns (total_ms over `steps` calls, per-call ms list, stats [B,H,2])."""
-    q, k, v, out, lse, stats = bufs
-    stream = torch.cuda.current_stream()
-    p = sa.make_params(lam=lam, stream=stream.cuda_stream, tile_q=cfg.tile if tile_k else 0, tile_k=tile_k,
-                       skip_mask_in=mask_in)
-    for _ in range(warmup):
-        sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p, mode, stats)
-    evs = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
-    barrier()
-    torch.cuda.synchronize()
-    if sampler is not None:
-        sampler.active.set()
-    evs[0].record(stream)
-    for i in range(steps):
-        sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p, mode, stats)
-        evs[i + 1].record(stream)
-    torch.cuda.synchronize()
-    if sampler is not None:
-        sampler.active.clear()
-    barrier()
-    per = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
-    return evs[0].elapsed_time(evs[-1]), per, stats.cpu().numpy().copy()
+def mode_entry(g, BH_total, ms, per, st_all, st_local):
+    cfg = g.cfg
+    ex = executed_flop(BH_total, cfg.N, cfg.D, st_all)
+    return {"ms": ms, "ms_min": float(np.min(per)), "ms_median": float(np.median(per)),
+            "sparsity": float(st_all[..., 1].sum() / st_all.sum()),
+            "effective_tflops": dense_flop(BH_total, cfg.N, cfg.D) / (ms * 1e-3) / 1e12,
+            "executed_tflops": ex / (ms * 1e-3) / 1e12,
+            "kernel_ms_avg_rank0": float(np.mean(per)),
+            "executed_flop_per_launch_rank0": executed_flop(g.B * g.H, cfg.N, cfg.D, st_local)}
 
 
 def time_reorder(sa, torch, cfg, brick, qkv, scratch_out, steps, warmup):
@@ -218,54 +318,178 @@ def time_reorder(sa, torch, cfg, brick, qkv, scratch_out, steps, warmup):
     return info, tuple(dst)
 
 
-def selector_comparison(sa, torch, bufs, cfg, lse_dense, out_dense, dyn, steps, warmup, barrier):
-    """the block-mask comparison methods of PAPER.md:61-62 through the same kernel.  Block mass of
-    the dense probabilities -> Top-K at DYNAMIC mode's tile budget and Top-P at DYNAMIC mode's mean recall -> MASK mode."""
-    q, k, v, out, lse, stats = bufs
+def timed_call(torch, fn, n, warm=2):
     stream = torch.cuda.current_stream()
+    for _ in range(warm):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(n):
+        fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n
+
+
+def selector_comparison(g, dyn, steps, warmup, theta_grid=(1e-7, 1e-6, 1e-5, 1e-4)):
+    """the block-mask comparison methods of PAPER.md:61-62 and the section-3 "ideal" mask
+     through the same kernel.  Block sums of p and p^2 of the dense probabilities -> Top-K at DYNAMIC
+    mode's tile budget, Top-P at DYNAMIC mode's mean recall, the greedy mask under Eq. 3 over a Theta grid -> MASK mode."""
+    sa, torch, cfg = g.sa, g.torch, g.cfg
+    st = g.stream.cuda_stream
     T = -(-cfg.N // cfg.tile)
-    mass = torch.empty((cfg.B, cfg.H, T, T), device="cuda", dtype=torch.float32)
-    bitmap = torch.empty((cfg.B, cfg.H, T, T), device="cuda", dtype=torch.uint8)
-
-    def timed(fn, n):
-        for _ in range(2):
-            fn()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record(stream)
-        for _ in range(n):
-            fn()
-        e1.record(stream)
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / n
-
-    ms_mass = timed(lambda: sa.sparse_attn_block_mass(q, k, lse_dense, mass, cfg.B, cfg.H, cfg.N, cfg.D, 0.0,
-                                                      stream.cuda_stream), max(3, steps // 2))
-    res = {"block_mass_ms": ms_mass,
-           "block_mass_tflops": 2.0 * cfg.B * cfg.H * cfg.N * cfg.N * cfg.D / (ms_mass * 1e-3) / 1e12,
+    mass = torch.empty((g.B, g.H, T, T), device="cuda", dtype=torch.float32)
+    sq = torch.empty_like(mass)
+    bitmap = torch.empty((g.B, g.H, T, T), device="cuda", dtype=torch.uint8)
+    n = max(3, steps // 4)
+    ms_mass = timed_call(torch, lambda: sa.sparse_attn_block_mass(g.q, g.k, g.lse_dense, mass, g.B, g.H, g.N, g.D, 0.0, st), n)
+    ms_stats = timed_call(torch, lambda: sa.sparse_attn_block_stats(g.q, g.k, g.lse_dense, mass, sq, g.B, g.H, g.N, g.D, 0.0, st), n)
+    qk_flop = 2.0 * g.B * g.H * g.N * g.N * g.D
+    res = {"block_mass_ms": ms_mass, "block_mass_tflops": qk_flop / (ms_mass * 1e-3) / 1e12,
+           "block_stats_ms": ms_stats, "block_stats_tflops": qk_flop / (ms_stats * 1e-3) / 1e12,
            "note": "mass and selection are a pre-pass the in-loop rule does not need (PAPER.md:109, :133)"}
-    for name, kind, param in (("topk_at_dynamic_budget", sa.SELECT_TOPK, max(1.0 - dyn["sparsity"], 1.0 / T)),
-                              ("topp_at_dynamic_recall", sa.SELECT_TOPP, min(max(dyn["recall_mean"], 0.01), 1.0))):
-        ms_sel = timed(lambda: sa.sparse_attn_select_blocks(mass, bitmap, cfg.B, cfg.H, T, T, kind, param,
-                                                            stream.cuda_stream), 3)
-        total, per, st = time_mode(sa, torch, bufs, cfg, sa.MODE_MASK, -math.inf, steps, warmup, barrier, None, 0, bitmap)
-        rec = torch.exp(lse - lse_dense)
-        err = (out.float() - out_dense.float()).abs()
-        res[name] = {"param": param, "select_ms": ms_sel, "attention_ms": total / steps,
-                     "sparsity": float(st[..., 1].sum() / st.sum()), "recall_min": float(rec.min()),
-                     "recall_mean": float(rec.mean()), "err_vs_dense_mean_abs": float(err.mean()),
-                     "ms_incl_prepass": total / steps + ms_mass + ms_sel}
+    jobs = [("topk_at_dynamic_budget", lambda: sa.sparse_attn_select_blocks(mass, bitmap, g.B, g.H, T, T, sa.SELECT_TOPK,
+                                                                            max(1.0 - dyn["sparsity"], 1.0 / T), st),
+             max(1.0 - dyn["sparsity"], 1.0 / T), ms_mass),
+            ("topp_at_dynamic_recall", lambda: sa.sparse_attn_select_blocks(mass, bitmap, g.B, g.H, T, T, sa.SELECT_TOPP,
+                                                                            min(max(dyn["recall_mean"], 0.01), 1.0), st),
+             min(max(dyn["recall_mean"], 0.01), 1.0), ms_mass)]
+    for theta in theta_grid:
+        jobs.append((f"greedy_eq3_theta_{theta:g}",
+                     (lambda th: lambda: sa.sparse_attn_select_blocks_greedy(mass, sq, bitmap, g.B, g.H, g.N, cfg.tile, T, th, st))(theta),
+                     theta, ms_stats))
+    for name, select, param, ms_pre in jobs:
+        ms_sel = timed_call(torch, select, 3, warm=1)
+        total, per, stt = g.time(sa.MODE_MASK, -math.inf, max(3, steps // 2), min(warmup, 2), mask_in=bitmap)
+        ms_att = total / max(3, steps // 2)
+        res[name] = {"param": param, "select_ms": ms_sel, "attention_ms": ms_att,
+                     "sparsity": float(stt[..., 1].sum() / stt.sum()), **g.quality(),
+                     "ms_incl_prepass": ms_att + ms_pre + ms_sel}
     return res
 
 
-def measured_hbm():
-    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(path):
-        with open(path) as f:
-            return float(json.load(f)["hbm_gbs"])
-    return 6650.0                                           # fallback stated in B200_PROFILING.md
+# ---------------------------------------------------------------------------------------------- reports (configs 2-4, masks)
+def sweep_point(g, mode, lam, steps, warmup, dense_ms, tile_k=0):
+    total, per, st = g.time(mode, lam, steps, warmup, tile_k=tile_k)
+    ms = total / steps
+    s = float(st[..., 1].sum() / st.sum())
+    return {"lambda": lam, "ms": ms, "sparsity": s, "speedup_vs_dense": dense_ms / ms, "mma_bound_model": 1.0 / (1.0 - s / 2.0),
+            **g.quality()}
 
 
+def report_cfg2(args, sa, torch):
+    """BASELINE.json configs[2]: per-head sparsity against (tau_h, sigma_h)."""
+    from workloads.generator import head_params
+    cfg = CONFIGS["cfg2"]
+    qb, kb, vb = make_qkv(cfg, args.seed, workers=host_workers())
+    g = Gpu(sa, torch, cfg, qb, kb, vb)
+    lam = eq7_lambda(cfg)
+    g.preheat(args.preheat)
+    total, per, _ = g.time(sa.MODE_DENSE, -math.inf, args.steps, args.warmup)
+    dense_ms = total / args.steps
+    g.keep_dense()
+    out = {"report": "cfg2", "workload": workload_name(cfg), "lambda": lam, "lambda_rule": f"Eq. 7, P_real={P_REAL}",
+           "dense_ms": dense_ms, "dense_tflops": dense_flop(cfg.H, cfg.N, cfg.D) / (dense_ms * 1e-3) / 1e12, "heads": []}
+    per_mode = {}
+    for mname, mode in (("fixed", sa.MODE_FIXED), ("dynamic", sa.MODE_DYNAMIC)):
+        out[mname] = sweep_point(g, mode, lam, args.steps, args.warmup, dense_ms)
+        st = g.stats.cpu().numpy()[0]
+        per_mode[mname] = [{"sparsity": float(st[h, 1] / st[h].sum()), **{k_: v_ for k_, v_ in g.quality((h, h + 1)).items()
+                                                                          if k_.startswith("recall")}} for h in range(cfg.H)]
+    taus, sigmas = zip(*(head_params(cfg, args.seed, h) for h in range(cfg.H)))
+    for h in range(cfg.H):
+        out["heads"].append({"head": h, "tau": taus[h], "sigma": sigmas[h],
+                             "fixed": per_mode["fixed"][h], "dynamic": per_mode["dynamic"][h]})
+    sp = np.array([e["sparsity"] for e in per_mode["dynamic"]])
+    out["dynamic_sparsity_corr_with_tau"] = float(np.corrcoef(sp, np.array(taus))[0, 1])
+    out["dynamic_sparsity_corr_with_sigma"] = float(np.corrcoef(sp, np.array(sigmas))[0, 1])
+    return out
+
+
+def report_cfg3(args, sa, torch):
+    """BASELINE.json configs[3]: recall-target sweep 0.85-0.99 (strict map, and the calibrated map of
+    SURVEY.md NEXT-3), the paper's lambda grid {-6,-8,-9,-11} (PAPER.md:212-217) and Eq. 7 with P_real in {0.5,1,1.5,3}
+    (PAPER.md:137-139): sparsity vs speed-up, DYNAMIC against FIXED, on the contract generator and the aligned variant."""
+    from paper_2606_16317_b200.calibrate import calibrate_lambda
+    out = {"report": "cfg3", "variants": {}}
+    targets = (0.85, 0.90, 0.95, 0.97, 0.99)
+    for name in ("cfg3", "cfg3_aligned"):
+        cfg = CONFIGS[name]
+        qb, kb, vb = make_qkv(cfg, args.seed, workers=host_workers())
+        g = Gpu(sa, torch, cfg, qb, kb, vb)
+        del qb, kb, vb
+        g.preheat(args.preheat)
+        total, per, _ = g.time(sa.MODE_DENSE, -math.inf, args.steps, args.warmup)
+        dense_ms = total / args.steps
+        g.keep_dense()
+        v = {"workload": workload_name(cfg), "dense_ms": dense_ms,
+             "dense_tflops": dense_flop(cfg.H, cfg.N, cfg.D) / (dense_ms * 1e-3) / 1e12, "sweeps": []}
+        modes = (("fixed", sa.MODE_FIXED), ("dynamic", sa.MODE_DYNAMIC))
+        for R in targets:
+            lam = math.log((1.0 - R) / cfg.N)
+            v["sweeps"].append({"rule": "strict map lambda = ln((1-R)/N)", "recall_target": R,
+                                **{m: sweep_point(g, mode, lam, args.steps, args.warmup, dense_ms) for m, mode in modes}})
+        for R in targets:
+            e = {"rule": "calibrated: largest lambda with MEAN row recall >= R (bisection, 12 iterations)", "recall_target": R}
+            for m, mode in modes:
+                cal = calibrate_lambda(g.q, g.k, g.v, cfg.B, cfg.H, cfg.N, cfg.D, mode, R, statistic="mean", iters=12)
+                e[m] = sweep_point(g, mode, cal["lambda"], args.steps, args.warmup, dense_ms)
+            v["sweeps"].append(e)
+        for lam in (-6.0, -8.0, -9.0, -11.0):
+            v["sweeps"].append({"rule": "paper lambda grid (Table 2)", "lambda": lam,
+                                **{m: sweep_point(g, mode, lam, args.steps, args.warmup, dense_ms) for m, mode in modes}})
+        for pr in (0.5, 1.0, 1.5, 3.0):
+            lam = eq7_lambda(cfg, p_real=pr)
+            v["sweeps"].append({"rule": "Eq. 7", "p_real": pr,
+                                **{m: sweep_point(g, mode, lam, args.steps, args.warmup, dense_ms) for m, mode in modes}})
+        out["variants"][name] = v
+        del g
+        torch.cuda.empty_cache()
+    return out
+
+
+def report_cfg4(args, sa, torch):
+    """BASELINE.json configs[4]: denoising-step drift sweep at the 720p shape, all 40 heads: X = (1-a) field + a noise."""
+    from paper_2606_16317_b200.calibrate import calibrate_lambda
+    cfg = CONFIGS["cfg4"]
+    lam = eq7_lambda(cfg)
+    out = {"report": "cfg4", "workload": workload_name(cfg), "lambda": lam, "lambda_rule": f"Eq. 7, P_real={P_REAL}", "sweep": []}
+    for a in (0.1, 0.3, 0.5, 0.7, 0.9):
+        qb, kb, vb = make_qkv(cfg, args.seed, noise_a=a, workers=host_workers())
+        g = Gpu(sa, torch, cfg, qb, kb, vb)
+        del qb, kb, vb
+        g.preheat(args.preheat)
+        total, per, _ = g.time(sa.MODE_DENSE, -math.inf, args.steps, args.warmup)
+        dense_ms = total / args.steps
+        g.keep_dense()
+        row = {"noise_a": a, "dense_ms": dense_ms}
+        for m, mode in (("fixed", sa.MODE_FIXED), ("dynamic", sa.MODE_DYNAMIC)):
+            row[m] = sweep_point(g, mode, lam, args.steps, args.warmup, dense_ms)
+            cal = calibrate_lambda(g.q, g.k, g.v, cfg.B, cfg.H, cfg.N, cfg.D, mode, 0.95, statistic="mean", iters=10)
+            row[m + "_at_mean_recall_0.95"] = sweep_point(g, mode, cal["lambda"], args.steps, args.warmup, dense_ms)
+        out["sweep"].append(row)
+        del g
+        torch.cuda.empty_cache()
+    return out
+
+
+def run_report(args):
+    import torch
+    import paper_2606_16317_b200 as sa
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (B200); there is no CPU fallback")
+    torch.cuda.set_device(0)
+    if args.report in ("masks", "kurtosis"):
+        from paper_2606_16317_b200 import analysis
+        fn = analysis.report_masks if args.report == "masks" else analysis.report_kurtosis
+        out = fn(args.seed)
+    else:
+        out = {"cfg2": report_cfg2, "cfg3": report_cfg3, "cfg4": report_cfg4}[args.report](args, sa, torch)
+    print(json.dumps(out), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -273,26 +497,38 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--seed", type=int, default=20261104)
-    ap.add_argument("--config", default="cfg1")
-    ap.add_argument("--no-aligned", action="store_true", help="skip the supplementary aligned workload")
+    ap.add_argument("--config", default=DEFAULT_CONFIG)
+    ap.add_argument("--no-aligned", action="store_true", help="skip the supplementary aligned / re-ordered workloads")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--preheat", type=float, default=1.5, help="seconds of untimed DENSE calls before each workload's timed modes")
     ap.add_argument("--modes", default="dense,fixed,dynamic", help="subset of modes to time (profiling runs)")
+    ap.add_argument("--report", default=None, choices=["cfg2", "cfg3", "cfg4", "masks", "kurtosis"],
+                    help="run one of the sweeps BASELINE.json configs[2..4] / SURVEY.md NEXT-4 ask for and print it as JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
     cfg = CONFIGS[args.config]
-    lam = math.log(P_REAL) + math.log(cfg.tile / cfg.N)        # Eq. 7
+    lam = eq7_lambda(cfg)
     if args.impl == "reference":
         run_reference(args, cfg, lam)
         return
-
-    import torch
-    import paper_2606_16317_b200 as sa   # raises if the CUDA extension is missing: no fallback
+    if args.report:
+        run_report(args)
+        return
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    # inputs first (spawned workers): weak scaling, every rank draws its own batch (different seed), same shape
+    workers = max(1, host_workers() // max(1, min(world, 8)))
+    host_data = {args.config: make_qkv(cfg, args.seed + 1000 * rank, workers=workers)}
+    aligned_name = args.config + "_aligned"
+    if not args.no_aligned and aligned_name in CONFIGS:
+        host_data[aligned_name] = make_qkv(CONFIGS[aligned_name], args.seed + 1000 * rank, workers=workers)
+
+    import torch
+    import paper_2606_16317_b200 as sa   # raises if the CUDA extension is missing: no fallback
+
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (B200); there is no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -308,74 +544,47 @@ def main():
 
     tb, ts, peak_kind = measured_peaks()
     BH = cfg.B * cfg.H
-
-    def to_dev(bits):
-        return torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
-
     results = {}
     # (result key, generator config, brick of the token re-ordering or None)
     variants = [(args.config, args.config, None)]
     if not args.no_aligned:
-        if args.config + "_aligned" in CONFIGS:
-            variants.append((args.config + "_aligned", args.config + "_aligned", None))
+        if aligned_name in host_data:
+            variants.append((aligned_name, aligned_name, None))
         # SURVEY.md 8(f) NEXT-1 / PAPER.md:139: the contract workload with its tokens re-ordered into bricks
         variants.append((args.config + "_brick%dx%dx%d" % BRICK, args.config, BRICK))
-    reorder_info = None
-    selectors = None
-    head_total_ms = None
+    reorder_info = selectors = head_total_ms = None
     sampler = ClockSampler(local_rank)
     sampler.__enter__()                     # clocks / throttle reasons are sampled inside every timed region below
-    launches0 = sa.launch_count()
     headline_launches = 0
+    want = args.modes.split(",")
     for vi, (name, gen_name, brick) in enumerate(variants):
         vcfg = CONFIGS[gen_name]
-        # weak scaling: every rank draws its own batch (different seed), same shape
-        if brick is None or gen_name != variants[0][1]:
-            qb, kb, vb = make_qkv(vcfg, args.seed + 1000 * rank)
-        else:
-            qb, kb, vb = keep_bufs                       # same bits as the contract workload
-        q, k, v = to_dev(qb), to_dev(kb), to_dev(vb)
-        out = torch.empty_like(q)
+        g = Gpu(sa, torch, vcfg, *host_data[gen_name], barrier=barrier)
         if brick is not None:
-            reorder_info, (q, k, v) = time_reorder(sa, torch, vcfg, brick, (q, k, v), out, args.steps, args.warmup)
-        lse = torch.empty((cfg.B, cfg.H, cfg.N), device="cuda", dtype=torch.float32)
-        stats = torch.zeros((cfg.B, cfg.H, 2), device="cuda", dtype=torch.int64)
-        bufs = (q, k, v, out, lse, stats)
-        # Untimed pre-heat: after the idle seconds of input generation the first timed mode would otherwise run at
-        # burst clocks and the later ones under the power cap, which biases every ratio between modes by a few percent.
-        t_heat = time.perf_counter()
-        p_heat = sa.make_params(stream=torch.cuda.current_stream().cuda_stream)
-        while time.perf_counter() - t_heat < args.preheat:
-            for _ in range(10):
-                sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D, p_heat, sa.MODE_DENSE, stats)
-            torch.cuda.synchronize()
+            reorder_info, (g.q, g.k, g.v) = time_reorder(sa, torch, vcfg, brick, (g.q, g.k, g.v), g.out, args.steps, args.warmup)
+        g.preheat(args.preheat)
         res = {}
-        lam32 = math.log(P_REAL) + math.log(32 / cfg.N)       # Eq. 7 with B_c = 32
+        lam32 = eq7_lambda(cfg, tile_k=32)                    # Eq. 7 with B_c = 32
         for mname, mode, mlam, mtk in (("dense", sa.MODE_DENSE, -math.inf, 0), ("fixed", sa.MODE_FIXED, lam, 0),
-                                       ("dynamic", sa.MODE_DYNAMIC, lam, 0),
-                                       ("dynamic_bc32", sa.MODE_DYNAMIC, lam32, 32),
+                                       ("dynamic", sa.MODE_DYNAMIC, lam, 0), ("dynamic_bc32", sa.MODE_DYNAMIC, lam32, 32),
                                        ("mask_replay", sa.MODE_MASK, lam, 0)):
+            mmask = None
             if mname == "mask_replay":
                 # MASK mode fed DYNAMIC mode's own decisions: same tiles, decisions read instead of taken in the loop
-                if args.no_aligned or "dynamic" not in res:
+                if args.no_aligned or "dynamic" not in res or vi != 1:
                     continue
                 T_dec = -(-cfg.N // cfg.tile)
-                replay_mask = torch.zeros((cfg.B, cfg.H, T_dec, T_dec), device="cuda", dtype=torch.uint8)
-                sa.sparse_attn_fwd(q, k, v, out, lse, cfg.B, cfg.H, cfg.N, cfg.D,
-                                   sa.make_params(lam=lam, skip_mask_out=replay_mask,
-                                                  stream=torch.cuda.current_stream().cuda_stream), sa.MODE_DYNAMIC, stats)
+                mmask = torch.zeros((cfg.B, cfg.H, T_dec, T_dec), device="cuda", dtype=torch.uint8)
+                g.call(sa.MODE_DYNAMIC, lam, skip_mask_out=mmask)
                 torch.cuda.synchronize()
-            elif mname.split("_")[0] not in args.modes.split(",") or (mtk and (args.no_aligned or cfg.D != 128)):
+            elif mname.split("_")[0] not in want or (mtk and (args.no_aligned or cfg.D != 128)):
                 continue
-            mmask = replay_mask if mname == "mask_replay" else None
             headline = (vi == 0 and mname == "dynamic")
+            l0 = sa.launch_count()
+            total, per, st = g.time(mode, mlam, args.steps, args.warmup, tile_k=mtk, mask_in=mmask, sampler=sampler)
             if headline:
-                l0 = sa.launch_count()
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk, mmask)
                 headline_launches = sa.launch_count() - l0 - args.warmup
                 head_total_ms = total
-            else:
-                total, per, st = time_mode(sa, torch, bufs, vcfg, mode, mlam, args.steps, args.warmup, barrier, sampler, mtk, mmask)
             if dist is not None:
                 t = torch.tensor([total], device="cuda")
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -385,38 +594,19 @@ def main():
                 st_all = gather_stats(torch.from_numpy(st).cuda(), cfg.H * world).cpu().numpy()[None]
             else:
                 st_all = st[None]
-            ms = total / args.steps
-            ex = executed_flop(BH * world, cfg.N, cfg.D, cfg.tile, st_all)
-            quality = {}
+            res[mname] = mode_entry(g, BH * world, total / args.steps, per, st_all, st[None])
             if mname == "dense":
-                out_dense, lse_dense = out.clone(), lse.clone()
-            elif "dense" in res:
-                # achieved recall per row = exp(lse_retained - lse_dense), error against dense
-                rec = torch.exp(lse - lse_dense)
-                err = (out.float() - out_dense.float()).abs()
-                quality = {"recall_min": float(rec.min()), "recall_mean": float(rec.mean()),
-                           "err_vs_dense_max_abs": float(err.max()), "err_vs_dense_mean_abs": float(err.mean())}
-                del rec, err
-            res[mname] = {
-                "ms": ms, "ms_min": float(np.min(per)), "ms_median": float(np.median(per)),
-                "sparsity": float(st_all[..., 1].sum() / st_all.sum()),
-                "effective_tflops": dense_flop(BH * world, cfg.N, cfg.D) / (ms * 1e-3) / 1e12,
-                "executed_tflops": ex / (ms * 1e-3) / 1e12,
-                "kernel_ms_avg_rank0": float(np.mean(per)),
-                "executed_flop_per_launch_rank0": executed_flop(BH, cfg.N, cfg.D, cfg.tile, st[None]),
-                **quality,
-            }
-        for mname in ("fixed", "dynamic", "dynamic_bc32", "mask_replay"):
-            if mname not in res or "dense" not in res:
-                continue
+                g.keep_dense()
+            else:
+                res[mname].update(g.quality())
             if mname == "dynamic_bc32":
                 res[mname]["lambda"] = lam32
                 res[mname]["decision_tile"] = "128x32"
-            res[mname]["speedup_vs_dense"] = res["dense"]["ms"] / res[mname]["ms"]
-            res[mname]["mma_bound_model"] = 1.0 / (1.0 - res[mname]["sparsity"] / 2.0)
-        if vi == 1 and brick is None and "dynamic" in res and "dense" in res and not args.no_aligned:
-            selectors = selector_comparison(sa, torch, bufs, vcfg, lse_dense, out_dense, res["dynamic"], args.steps,
-                                            args.warmup, barrier)
+            if mname != "dense" and "dense" in res:
+                res[mname]["speedup_vs_dense"] = res["dense"]["ms"] / res[mname]["ms"]
+                res[mname]["mma_bound_model"] = 1.0 / (1.0 - res[mname]["sparsity"] / 2.0)
+        if vi == 1 and brick is None and "dynamic" in res and "dense" in res:
+            selectors = selector_comparison(g, res["dynamic"], args.steps, args.warmup)
         if brick is not None and reorder_info is not None:
             for mname in ("fixed", "dynamic", "dynamic_bc32"):
                 if mname in res and "dense" in results.get(variants[0][0], {}):
@@ -425,17 +615,14 @@ def main():
                     res[mname]["speedup_vs_plain_dense_incl_reorder"] = (
                         results[variants[0][0]]["dense"]["ms"] / res[mname]["ms_with_reorder"])
         results[name] = res
-        if vi == 0:
-            keep_bufs = (qb, kb, vb)
-        out_dense = lse_dense = None
-        del q, k, v, out, lse, stats, bufs
+        del g
         torch.cuda.empty_cache()
 
     sampler.__exit__()
     clocks = sampler.summary()
 
     # ------------------------------------------------------------------ end-to-end through the host-buffer C entry point
-    qb, kb, vb = keep_bufs
+    qb, kb, vb = host_data[args.config]
     hq, hk, hv = (torch.from_numpy(x.view(np.int16)).pin_memory() for x in (qb, kb, vb))
     hout = torch.empty_like(hq).pin_memory()
     hlse = torch.empty((cfg.B, cfg.H, cfg.N), dtype=torch.float32).pin_memory()
@@ -467,44 +654,51 @@ def main():
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
         r = oracle_sample_time(cfg, args.seed, lam, 2)
-        cpu_baseline = {"value": r["flop"] / r["seconds"][0] / 1e12, "unit": "TFLOP/s (dense-equivalent, effective)",
+        cpu_baseline = {"value": r["flop"] / r["seconds"][0] / 1e12, "unit": UNIT,
                         "cores": r["cores"], "kind": "oracle", "sample": r["sample"], "seconds": r["seconds"][0],
                         "extrapolated_full_config_seconds": r["seconds"][0] * dense_flop(BH, cfg.N, cfg.D) / r["flop"]}
 
-    if set(args.modes.split(",")) != {"dense", "fixed", "dynamic"}:      # profiling run: raw numbers only
+    if set(want) != {"dense", "fixed", "dynamic"}:      # profiling run: raw numbers only
         print(json.dumps({"partial": True, "modes": results, "lambda": lam}), flush=True)
         return
     main_res = results[args.config]["dynamic"]
     dense_res = results[args.config]["dense"]
-    # roofline of the dominant (only) kernel, in the mode with the most executed work per launch: DENSE
-    ach = dense_res["executed_flop_per_launch_rank0"] / (dense_res["kernel_ms_avg_rank0"] * 1e-3) / 1e12
+    # Roofline of the dominant (only) kernel IN THE HEADLINE LAUNCH (DYNAMIC mode): executed FLOP of that launch (Q K^T for
+    # every tile + P V for the executed ones, from stats_out) / its own CUDA-event time; the same kernel's DENSE launch beside it.
     ach_dyn = main_res["executed_flop_per_launch_rank0"] / (main_res["kernel_ms_avg_rank0"] * 1e-3) / 1e12
+    ach_dense = dense_res["executed_flop_per_launch_rank0"] / (dense_res["kernel_ms_avg_rank0"] * 1e-3) / 1e12
+    traffic, traffic_src = ncu_traffic(args.config, "dynamic")
+    alg_bytes = 4 * BH * cfg.N * cfg.D * 2 + BH * cfg.N * 4
     line = {
         "metric": METRIC,
         "value": main_res["effective_tflops"],
-        "unit": "TFLOP/s (dense-equivalent attention FLOP / time, DYNAMIC mode)",
+        "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": head_total_ms / args.steps if world == 1 else main_res["ms"],
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "mode": "dynamic", "lambda": lam,
-                   "lambda_rule": f"Eq. 7, P_real={P_REAL}", "l2": "q+k+v+out = 805 MB per step > 126 MB L2, no flush",
+                   "lambda_rule": f"Eq. 7, P_real={P_REAL}",
+                   "l2": "q+k+v+out = %.0f MB per step > 126 MB L2, no flush" % (4 * BH * cfg.N * cfg.D * 2 / 1e6),
                    "preheat_s": args.preheat,
                    "parallelism": f"heads sharded, {world} rank(s), no data-path collective"},
         "sparsity_pct": 100.0 * main_res["sparsity"],
         "speedup_vs_dense": main_res["speedup_vs_dense"],
-        "pct_tensor_peak_executed": {"dense": 100.0 * ach / tb, "dynamic": 100.0 * ach_dyn / tb,
+        "pct_tensor_peak_executed": {"dense": 100.0 * ach_dense / tb, "dynamic": 100.0 * ach_dyn / tb,
                                      "of": f"{tb} TFLOP/s ({peak_kind} burst)"},
         "modes": results,
-        "roofline": {"bound": "tensor", "achieved": ach, "peak": tb, "unit": "TFLOP/s", "frac": ach / tb,
-                     "traffic": NCU_DRAM_BYTES_DENSE_CFG1 if args.config == "cfg1" else None, "kernel": "sparse_attn_fwd_kernel<128,128,1,*> DENSE mode",
-                     "peak_kind": f"{peak_kind} bf16 burst; sustained {ts}", "frac_sustained": ach / ts,
-                     "frac_dynamic_mode": ach_dyn / tb,
-                     "flop_per_launch": dense_res["executed_flop_per_launch_rank0"],
-                     "launch_ms": dense_res["kernel_ms_avg_rank0"]},
+        "roofline": {"bound": "tensor", "achieved": ach_dyn, "peak": tb, "unit": "TFLOP/s", "frac": ach_dyn / tb,
+                     "traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes": alg_bytes,
+                     "kernel": "sparse_attn_fwd_kernel<128,128,1,3,2,true,false,1>, DYNAMIC mode (the headline launch)",
+                     "peak_kind": f"{peak_kind} bf16 burst; sustained {ts}", "frac_sustained": ach_dyn / ts,
+                     "flop_per_launch": main_res["executed_flop_per_launch_rank0"],
+                     "launch_ms": main_res["kernel_ms_avg_rank0"],
+                     "frac_dense": ach_dense / tb, "frac_dense_sustained": ach_dense / ts,
+                     "dense_flop_per_launch": dense_res["executed_flop_per_launch_rank0"],
+                     "dense_launch_ms": dense_res["kernel_ms_avg_rank0"]},
         "cpu_baseline": cpu_baseline,
-        "e2e": {"value": dense_flop(BH * world, cfg.N, cfg.D) / e2e_s / 1e12,
-                "unit": "TFLOP/s (dense-equivalent, host buffers, H2D + kernel + D2H)",
-                "ms_per_step": e2e_s * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "e2e": {"value": dense_flop(BH * world, cfg.N, cfg.D) / e2e_s / 1e12, "unit": UNIT,
+                "ms_per_step": e2e_s * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "path": "sparse_attn_fwd_host: pinned host buffers, H2D + kernel + D2H pipelined over head chunks"},
         "token_reordering": reorder_info,
         "block_selectors_on_aligned_workload": selectors,
         "gpu_launches": headline_launches,

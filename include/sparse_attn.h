@@ -213,6 +213,19 @@ int sparse_attn_select_blocks(const float* mass, uint8_t* skip_mask_out, int B, 
 int sparse_attn_select_blocks_greedy(const float* mass, const float* sqmass, uint8_t* skip_mask_out, int B, int H, int N,
                                      int tile_q, int T_c, double theta, void* stream);
 
+/*
+ * Quality of a sparse run against the dense run of the same inputs, reduced on the device (harness support; the
+ * paper's quality measures: recall = kept share of the softmax mass, and |O - O'|).
+ *
+ * sparse_attn_recall_stats: recall_r = e^{lse_retained[r] - lse_dense[r]} for n_rows rows (both device fp32, natural
+ *   log, as sparse_attn_fwd writes them); stats_out (DEVICE, double[2]) = {min_r recall_r, sum_r recall_r}.
+ * sparse_attn_output_error: stats_out (DEVICE, double[2]) = {max |a - b|, sum |a - b|} over n_elems bf16 elements
+ *   (n_elems even, buffers 4-byte aligned), e.g. a sparse output against the dense one.
+ * Each enqueues two small kernels on `stream` and returns; the caller synchronises before reading stats_out.
+ */
+int sparse_attn_recall_stats(const float* lse_retained, const float* lse_dense, int64_t n_rows, double* stats_out, void* stream);
+int sparse_attn_output_error(const void* out_a, const void* out_b, int64_t n_elems, double* stats_out, void* stream);
+
 /* Static string for a status code. */
 const char* sparse_attn_status_string(int status);
 

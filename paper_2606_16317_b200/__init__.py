@@ -25,6 +25,8 @@ from .binding import (  # noqa: F401
     sparse_attn_fwd,
     sparse_attn_fwd_host,
     sparse_attn_reorder_tokens,
+    sparse_attn_output_error,
+    sparse_attn_recall_stats,
     sparse_attn_select_blocks,
     sparse_attn_select_blocks_greedy,
     status_string,

@@ -27,6 +27,8 @@ EXPORTED_SYMBOLS = (
     "sparse_attn_block_mass",
     "sparse_attn_block_stats",
     "sparse_attn_select_blocks_greedy",
+    "sparse_attn_recall_stats",
+    "sparse_attn_output_error",
     "sparse_attn_brick_permutation",
     "sparse_attn_reorder_tokens",
     "sparse_attn_select_blocks",
@@ -87,6 +89,10 @@ def _load():
         lib.sparse_attn_block_stats.argtypes = [ctypes.c_void_p] * 5 + [ctypes.c_int] * 4 + [ctypes.c_float, ctypes.c_void_p]
         lib.sparse_attn_select_blocks_greedy.restype = ctypes.c_int
         lib.sparse_attn_select_blocks_greedy.argtypes = [ctypes.c_void_p] * 3 + [ctypes.c_int] * 5 + [ctypes.c_double, ctypes.c_void_p]
+        lib.sparse_attn_recall_stats.restype = ctypes.c_int
+        lib.sparse_attn_recall_stats.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sparse_attn_output_error.restype = ctypes.c_int
+        lib.sparse_attn_output_error.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
         lib.sparse_attn_select_blocks.restype = ctypes.c_int
         lib.sparse_attn_select_blocks.argtypes = [ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 5 + [
             ctypes.c_double, ctypes.c_void_p]
@@ -219,6 +225,22 @@ def sparse_attn_select_blocks_greedy(mass, sqmass, skip_mask_out, B, H, N, tile_
     """C entry point `sparse_attn_select_blocks_greedy` (device buffers): the section-3 mask under Eq. 3's bound."""
     rc = _load().sparse_attn_select_blocks_greedy(_ptr(mass), _ptr(sqmass), _ptr(skip_mask_out), int(B), int(H), int(N),
                                                   int(tile_q), int(T_c), float(theta), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_recall_stats(lse_retained, lse_dense, n_rows, stats_out, stream=None):
+    """C entry point `sparse_attn_recall_stats`: stats_out (device double[2]) = {min, sum} of e^(lse_retained - lse_dense)."""
+    rc = _load().sparse_attn_recall_stats(_ptr(lse_retained), _ptr(lse_dense), int(n_rows), _ptr(stats_out), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_output_error(out_a, out_b, n_elems, stats_out, stream=None):
+    """C entry point `sparse_attn_output_error`: stats_out (device double[2]) = {max, sum} of |a - b| over bf16 elements."""
+    rc = _load().sparse_attn_output_error(_ptr(out_a), _ptr(out_b), int(n_elems), _ptr(stats_out), _ptr(stream))
     if rc != 0:
         raise SparseAttnError(rc, last_error())
     return rc

@@ -4,7 +4,8 @@ The paper compares methods at equal quality; on inputs where the worst-case map 
 skips nothing, the informative comparison is at equal ACHIEVED recall.  Recall costs nothing extra:
 for every row r, recall_r = exp(lse_retained_r - lse_dense_r), the share of the softmax mass the
 retained tiles hold.  This module bisects lambda until a statistic of recall (min or mean over rows)
-meets a target.  Harness logic only: every attention call goes through `sparse_attn_fwd`.
+meets a target.  Harness logic only: every attention call goes through `sparse_attn_fwd` and the recall
+statistic through `sparse_attn_recall_stats`; torch provides device memory and the stream, no arithmetic.
 """
 from __future__ import annotations
 
@@ -51,6 +52,7 @@ def calibrate_lambda(q, k, v, B, H, N, D, mode, target: float, statistic: str = 
     lse_d = torch.empty((B, H, N), device=q.device, dtype=torch.float32)
     lse = torch.empty_like(lse_d)
     stats = torch.zeros((B, H, 2), device=q.device, dtype=torch.int64)
+    rstats = torch.zeros(2, device=q.device, dtype=torch.float64)
     sa.sparse_attn_fwd(q, k, v, out, lse_d, B, H, N, D, sa.make_params(stream=st), sa.MODE_DENSE, stats)
     last = {}
     calls = [1]
@@ -59,10 +61,11 @@ def calibrate_lambda(q, k, v, B, H, N, D, mode, target: float, statistic: str = 
         upper = min(lam, 0.0) if mode == sa.MODE_FIXED else lam
         sa.sparse_attn_fwd(q, k, v, out, lse, B, H, N, D, sa.make_params(lam=upper, stream=st), mode, stats)
         calls[0] += 1
-        rec = torch.exp(lse - lse_d)
-        s = stats.sum(dim=(0, 1)).tolist()
-        last[lam] = {"lambda": lam, "recall_min": float(rec.min()), "recall_mean": float(rec.mean()),
-                     "sparsity": s[1] / max(s[0] + s[1], 1)}
+        sa.sparse_attn_recall_stats(lse, lse_d, B * H * N, rstats, st)
+        rmin, rsum = rstats.tolist()                       # (.tolist() synchronises)
+        executed, skipped = (sum(col) for col in zip(*stats.reshape(-1, 2).tolist()))
+        last[lam] = {"lambda": lam, "recall_min": rmin, "recall_mean": rsum / (B * H * N),
+                     "sparsity": skipped / max(executed + skipped, 1)}
         return last[lam]["recall_" + statistic]
 
     lam, _ = bisect_lambda(recall_at, target, lo, hi, iters)

@@ -8,14 +8,14 @@
 //   warps 0-3   softmax warpgroup of slot 0 (thread <-> query row <-> TMEM lane)
 //   warps 4-7   softmax warpgroup of slot 1
 //   warp  8     TMA producer for Q (once) and the K ring (runs ahead of the decisions)
-//   warp  9     tcgen05.mma issuer of slot 0 (of both slots in DENSE mode; one elected lane) and TMEM owner
+//   warp  9     tcgen05.mma issuer of slot 0 (one elected lane) and TMEM owner
 //   warp  10    TMA producer for the V ring: slot j % NV holds V_j.  DENSE: every tile.  Sparse modes: this warp
 //               reads both slots' votes on tile j and fetches V_j only if some slot keeps tile j (plus V_{j+1}
 //               speculatively after a kept tile); an unneeded tile completes its ring phase without a load
-//   warp  11    tcgen05.mma issuer of slot 1 in the sparse modes (idle in DENSE mode)
-// One issuer warp per slot in the sparse modes: a thread that issues tcgen05.mma is held until its last MMA has been
-// dispatched to the tensor pipe, so with a single issuer every barrier wait and vote decode of one slot left the pipe
-// idle; with two, the control work of one slot overlaps the MMAs of the other.
+//   warp  11    tcgen05.mma issuer of slot 1
+// One issuer warp per slot: a thread that issues tcgen05.mma is held until its last MMA has been dispatched to the
+// tensor pipe, so with a single issuer every barrier wait and vote decode of one slot left the pipe idle; with two,
+// the control work of one slot overlaps the MMAs of the other.
 // TMEM (512 columns): S_0 | S_1 (fp32, BC columns each; P_X, bf16x2, aliases the first BC/2 columns of S_X)
 //                     O_0 | O_1 (fp32, D columns each).
 // Per slot X and K tile j:  S_X = Q_X K_j^T (always)  ->  softmax warpgroup: row max, skip predicate,
@@ -53,11 +53,10 @@ constexpr float kRescaleThreshold = 8.0f;
 // Of every 16 pairs of logits (one 32-column chunk), this many take their exponential on the FMA pipe (range
 // reduction + cubic, packed f32x2) instead of MUFU.EX2: the MUFU pipe (16 / clk / SM) needs exactly as long for the
 // N^2 exponentials as the tensor pipe for the MMAs, so every exponential moved off it shortens the softmax phase.
-#ifndef DSA_POLY_PAIRS
-#define DSA_POLY_PAIRS 0
-#endif
-constexpr int kPolyPairs = DSA_POLY_PAIRS;
-static_assert(kPolyPairs == 0 || kPolyPairs == 1 || kPolyPairs == 2 || kPolyPairs == 4 || kPolyPairs == 8 || kPolyPairs == 16, "pairs per chunk on the FMA pipe");
+// Measured on config 1 (steady clocks): 0 / 2 / 3 / 4 of 16 -> DENSE 10.54 / 10.30 / 10.28 / 10.28 ms, FIXED 10.79 / 10.22 /
+// 10.44 / 10.52 ms; 8 of 16 is slower than none (issue slots).
+constexpr int kPolyPairs = 2;
+static_assert(kPolyPairs >= 0 && kPolyPairs <= 16, "pairs per chunk on the FMA pipe");
 
 struct FwdArgs {
     __nv_bfloat16* out;          // [BH, N, D]
@@ -96,17 +95,17 @@ struct SmemLayout {
     // base address per slot, which the softmax threads keep in a register for the whole K loop.
     static constexpr int kSlotOff = kMiscOff + 16;
     static constexpr int kSFull = 0;        // S_X(j) complete in TMEM                                  (count 1)
-    static constexpr int kPHalf = 8;        // first half of P_X written (kept tiles only)             (count 128)
-    static constexpr int kPReady = 16;      // all of P_X written (kept tiles only)                    (count 128)
-    static constexpr int kOFull = 24;       // last P V of slot X complete                             (count 1)
-    static constexpr int kSRead = 32;       // the 4 warps of slot X hold S_X(j) in registers          (count 4)
-    static constexpr int kDec = 48;         // dec[4]: the 4 warps of slot X have voted on tile j      (count 4), ring j & 3
-    static constexpr int kVotes = 80;       // votes[4][4]: (j << 2) | vote of warp w on tile j, ring j & 3, 16-B rows
-    static constexpr int kWmax = 144;       // wmax[4][4]: per-warp max of t (debug margins), ring j & 3
-    static constexpr int kPvMask = 208;     // pvmask[4]: kept sub-tiles of tile j (SUB > 1), ring j & 3
-    static constexpr int kPre = 224;        // pre[5][4] (SUB > 1): per-warp sub-tile votes: groups 0, 1 the preliminary
+    static constexpr int kPReady = 8;       // all of P_X written (kept tiles only)                    (count 128)
+    static constexpr int kOFull = 16;       // last P V of slot X complete                             (count 1)
+    static constexpr int kSRead = 24;       // the 4 warps of slot X hold S_X(j) in registers          (count 4)
+    static constexpr int kPPart = 32;       // p_part[3]: the first 1, 2, 3 parts of P_X written (kept tiles only; count 128)
+    static constexpr int kDec = 56;         // dec[4]: the 4 warps of slot X have voted on tile j      (count 4), ring j & 3
+    static constexpr int kVotes = 96;       // votes[4][4]: (j << 2) | vote of warp w on tile j, ring j & 3, 16-B rows
+    static constexpr int kWmax = 160;       // wmax[4][4]: per-warp max of t (debug margins), ring j & 3
+    static constexpr int kPvMask = 224;     // pvmask[4]: kept sub-tiles of tile j (SUB > 1), ring j & 3
+    static constexpr int kPre = 240;        // pre[5][4] (SUB > 1): per-warp sub-tile votes: groups 0, 1 the preliminary
                                             // round of tile j (by parity), groups 2..4 the later rounds of sub-tiles 1..3
-    static constexpr int kSlotStride = 304;
+    static constexpr int kSlotStride = 320;
     static constexpr int kTotal = kSlotOff + 2 * kSlotStride;
     static constexpr int kDynamicBytes = kTotal + 1024;  // slack for the 1024-B alignment of the swizzled tiles
     static_assert(kSlotOff % 16 == 0 && kSlotStride % 16 == 0, "vote rows are read with 16-byte loads");
@@ -140,7 +139,7 @@ __device__ __forceinline__ void exp_chunk(const uint32_t (&s)[32], uint64_t scal
     for (int i = 0; i < 16; ++i) {
         const uint64_t X = fma_f32x2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), scale2, negm2);
         float p0, p1;
-        if (kPolyPairs > 0 && (i % (16 / (kPolyPairs > 0 ? kPolyPairs : 1))) == (16 / (kPolyPairs > 0 ? kPolyPairs : 1)) - 1) {
+        if (((i + 1) * kPolyPairs) / 16 > (i * kPolyPairs) / 16) {              // kPolyPairs of the 16 pairs, evenly spread
             exp2_poly_x2(X, p0, p1);
         } else {
             float x0, x1;
@@ -173,6 +172,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                   (kSparse && G == 1 && (SUB == 2 || SUB == 4) && (BC / kSubN) % 32 == 0), "sub-tile decisions / mass kernel");
     constexpr int BR = 128 / G;
     constexpr int kSubD = D / 64;
+    // P_X is handed to the issuer in kHand parts of BC / kHand keys, so that the P V steps of a part run while the next
+    // part is exponentiated and only the last part's steps follow the last exponential
+    constexpr int kHand = (SUB == 1 && BC / 32 >= 4) ? 4 : 2;
     constexpr uint32_t kIdescQK = umma_idesc_bf16(128, BC, 0);   // S = Q K^T: A, B both K-major
     constexpr uint32_t kIdescPV = umma_idesc_bf16(128, D, 1);    // O += P V: B = V is MN-major (d contiguous)
 
@@ -215,7 +217,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             const uint32_t sb = slot(x);
             mbar_init(q_full(x), 1);
             mbar_init(sb + L::kSFull, 1);
-            mbar_init(sb + L::kPHalf, 128);
+            for (int h = 0; h < 3; ++h) mbar_init(sb + L::kPPart + 8 * h, 128);
             mbar_init(sb + L::kPReady, 128);
             mbar_init(sb + L::kOFull, 1);
             mbar_init(sb + L::kSRead, 4);
@@ -319,9 +321,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
         } else if (warp == kMmaWarp0 || warp == kMmaWarp1) {
             // ========================================================== MMA issuer(s) (a2, a6)
-            // kIssuers == 2: warp 9 drives slot 0 and warp 11 slot 1.  kIssuers == 1: warp 9 drives both slots in turn
-            // (warp 11 idles), which forces the two slots into anti-phase -- the best schedule when every tile is kept.
-            constexpr int kIssuers = kSparse ? 2 : 1;
+            // kIssuers == 2: warp 9 drives slot 0 and warp 11 slot 1 (every mode; measured on config 1: DENSE 10.16 ms with
+            // two issuers and the gate below against 10.32 ms with one issuer driving both slots in turn; without the
+            // gate 11.8 ms).  The single-issuer path (kIssuers == 1, warp 11 idle) is kept for comparison.
+            constexpr int kIssuers = 2;
             constexpr bool kGate = kIssuers == 2;
             const int x_lo = (kIssuers == 2 && warp == kMmaWarp1) ? 1 : 0;
             const int x_hi = (kIssuers == 2) ? x_lo + 1 : nX;        // this warp drives slots [x_lo, x_hi)
@@ -335,10 +338,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             umma_smem_desc_sw128(kaddr + koff, 16, 1024), kIdescQK, kk > 0);
                 }
             };
-            // half 0 / 1: keys [0, BC/2) / [BC/2, BC); mask (SUB > 1): bit s set = decision sub-tile s was kept
-            auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int half, uint32_t mask = 0xffu) {
+            // part h of kHand: keys [h BC / kHand, (h + 1) BC / kHand); mask (SUB > 1): bit s set = decision sub-tile s was kept
+            auto issue_pv = [&](int x, uint32_t vaddr, bool acc, int part, uint32_t mask = 0xffu) {
 #pragma unroll
-                for (int kk = half * (BC / 32); kk < (half + 1) * (BC / 32); ++kk) {
+                for (int kk = part * (BC / 16 / kHand); kk < (part + 1) * (BC / 16 / kHand); ++kk) {
                     if (SUB > 1 && !((mask >> (kk / (BC / 16 / kSubN))) & 1u)) continue;   // P of a skipped sub-tile is never read
                     // 16 keys = 16 rows of 128 B; d sub-tiles (64 columns) are L::kSubKVBytes apart (LBO)
                     umma_ts(tmem_base + 2 * BC + x * D, tmem_base + x * BC + kk * 8,
@@ -405,20 +408,23 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         while (static_cast<int>(ld_shared_u32(prog0 + 4 * (1 - x))) < need) { }
                     }
                     if (keep) {
-                        mbar_wait(sb + L::kPHalf, ppar[x]);
-                        mbar_wait(v_full(vslot), vph);       // V_j has landed (sparse modes: fetched by the V warp
-                        tc_fence_after();                    // once some slot voted to keep tile j, or prefetched)
-                        uint32_t pvmask = 0xffu;
-                        if (SUB > 1) pvmask = ld_shared_u32(sb + L::kPvMask + 4 * (j & 3));
-                        if (elect_one_sync()) issue_pv(x, vaddr, j > 0, 0, pvmask);
-                        __syncwarp();
+#pragma unroll
+                        for (int h = 0; h < kHand - 1; ++h) {
+                            mbar_wait(sb + L::kPPart + 8 * h, ppar[x]);
+                            if (h == 0) mbar_wait(v_full(vslot), vph);   // V_j has landed (sparse modes: fetched by the V warp
+                            tc_fence_after();                            // once some slot voted to keep tile j, or prefetched)
+                            uint32_t pvmask = 0xffu;
+                            if (SUB > 1) pvmask = ld_shared_u32(sb + L::kPvMask + 4 * (j & 3));
+                            if (elect_one_sync()) issue_pv(x, vaddr, j > 0 || h > 0, h, pvmask);
+                            __syncwarp();
+                        }
                         mbar_wait(sb + L::kPReady, ppar[x]);
                         tc_fence_after();
                         ppar[x] ^= 1u;
                         uint32_t pvmask2 = 0xffu;            // the mask is complete once all of P_x has been handed over
                         if (SUB > 1) pvmask2 = ld_shared_u32(sb + L::kPvMask + 4 * (j & 3));
                         if (elect_one_sync()) {
-                            issue_pv(x, vaddr, true, 1, pvmask2);
+                            issue_pv(x, vaddr, true, kHand - 1, pvmask2);
                             umma_commit(v_empty(vslot));     // this slot's P_x V_j has read V_j
                             if (has_next) {
                                 issue_qk(x, kaddr);          // (again, if a speculative one was overwritten by P_x)
@@ -478,8 +484,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         // (which put ~60 instructions between the row max and the first exponential of a retained tile).
         uint32_t sb = slot(x);
         uint32_t vote_w = sb + L::kVotes + 4 * w;
-        asm volatile("" : "+r"(sb), "+r"(vote_w));
-        uint32_t kst = 0;                                    // K stage of tile j (w == 0 releases it)
+        uint32_t kst = k_empty(0);                           // k_empty of the K stage of tile j (warp 0, lane 0 releases it)
+        asm volatile("" : "+r"(sb), "+r"(vote_w), "+r"(kst));
+        const bool lane0 = lane == 0;
+        const bool k_releaser = w == 0 && lane == 0;
 
         // MASS mode: -lse_r in log2 units (rows beyond N contribute nothing)
         float neg_lse2 = -INFINITY;
@@ -508,19 +516,19 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             mbar_wait(sb + L::kSFull, sfpar);
             sfpar ^= 1u;
             tc_fence_after();
-            // S_x(j) is complete, so this slot's Q K^T has read K_j for the last time (a mis-speculated S_x(j) was
-            // consumed, and issued again, during tile j-1): release this slot's hold on the K stage
-            if (w == 0 && lane == 0) mbar_arrive(k_empty(0) + 8 * kst);
-            if (++kst == NK) kst = 0;
             uint32_t su[BC / 32][32];                         // this thread's row of S_ij (fp32 bits)
 #pragma unroll
             for (int c = 0; c < BC / 32; ++c) tmem_ld_x32(tS + c * 32, su[c]);
+            // (under the TMEM loads) S_x(j) is complete, so this slot's Q K^T has read K_j for the last time (a
+            // mis-speculated S_x(j) was consumed, and issued again, during tile j-1): release this slot's hold on the K stage
+            mbar_arrive_if(kst, k_releaser);
+            kst = (kst == k_empty(NK - 1)) ? k_empty(0) : kst + 8;
             tmem_wait_ld();
             // inside a run of skipped tiles the MMA warp issues S_x(j+1) as soon as S_x(j) has left TMEM
             const bool spec = kSparse && prev_skip && (j + 1) < T_c;
             if (kSparse) {                                   // S_x(j) has left TMEM
                 tc_fence_before();
-                if (lane == 0) mbar_arrive(sb + L::kSRead);
+                mbar_arrive_if(sb + L::kSRead, lane0);
             }
 #define S_AT(c) __uint_as_float(su[(c) >> 5][(c) & 31])
             const int valid_cols = a.N - j * BC;             // ragged last K tile: columns beyond N are -inf
@@ -775,7 +783,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
                         tmem_wait_st();
                         tc_fence_before();
-                        mbar_arrive(sb + L::kPHalf);
+                        mbar_arrive(sb + L::kPPart);
                         half_sent = true;
                     }
                 }
@@ -792,28 +800,25 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
                 tmem_wait_st();
                 tc_fence_before();
-                if (!half_sent) mbar_arrive(sb + L::kPHalf); // (release: the mask above is visible to the issuer)
+                if (!half_sent) mbar_arrive(sb + L::kPPart); // (release: the mask above is visible to the issuer)
                 mbar_arrive(sb + L::kPReady);
                 fold();                                      // statistics for the next tile, behind the hand-over
                 continue;
             }
             // ---- predicate and all-rows vote (a4)
-            bool skip_grp = false, keep_any = true;
-            float grp_margin = INFINITY;
+            bool skip_grp = false, keep_any = true, wskip = false;
             if (kSparse) {
                 // votes[j & 3][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
                 // The MMA warp combines the four votes itself (barrier dec, one arrival per warp), so an all-skip
                 // decision reaches the tensor pipe without the four warps first synchronising with each other.
                 const bool row_skip = mhat2 < thr;           // Eq. 5 against this row's threshold (false at j = 0)
-                const bool wskip = __all_sync(0xffffffffu, row_skip);
+                wskip = __all_sync(0xffffffffu, row_skip);
                 const uint32_t q16 = static_cast<uint32_t>(j & 3) << 4;
                 tc_fence_before();                           // S_x(j) is in registers: the MMA warp may overwrite it
-                if (lane == 0) {
-                    st_shared_u32(vote_w + q16, static_cast<uint32_t>((j << 2) | (wskip ? 1 : 2)));
-                    mbar_arrive(sb + L::kDec + (q16 >> 1));
-                }
-                __syncwarp();
+                st_shared_u32_if(vote_w + q16, static_cast<uint32_t>((j << 2) | (wskip ? 1 : 2)), lane0);
+                mbar_arrive_if(sb + L::kDec + (q16 >> 1), lane0);
                 if (kDebug) {
+                    float grp_margin = INFINITY;
                     const uint32_t wm = sb + L::kWmax + q16;
                     if (want_margin) {
                         const float ref = (mode == kModeFixed) ? m_true : lse2;
@@ -843,9 +848,24 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         if (a.skip_mask) a.skip_mask[tile_row + j] = skip_grp ? 1 : 0;
                         if (want_margin) a.margin[tile_row + j] = grp_margin;
                     }
-                } else if (wskip) {
+                    wskip = false;                           // (settled above)
+                }
+            } else if (kDebug && grp_leader && grp_valid) {  // DENSE: nothing is skipped, every margin is +inf
+                if (a.skip_mask) a.skip_mask[tile_row + j] = 0;
+                if (want_margin) a.margin[tile_row + j] = INFINITY;
+            }
+            // ---- online softmax update (a5), first part.  A retained tile of a warp with a keeping row, outside a skip run
+            // and with no row whose max grew past the lazy-rescale gate -- the common case -- takes none of the branches
+            // below: one test covers the three rare events.  The first retained tile takes the rescale path too (m_used =
+            // m_gate = -inf: alpha = 0, l = 0 stays 0; O, still unwritten, is overwritten by the non-accumulating P V of
+            // tile 0), which spares a j == 0 test.
+            const bool need = mhat2 > m_gate;
+            const bool need_any = __any_sync(0xffffffffu, need);
+            if (__builtin_expect(wskip || spec || need_any || (kSparse && kDebug), 0)) {
+                if (wskip) {
                     // every row of this warp is below the threshold: wait (hardware-suspended, no shared-memory
                     // polling) until all four warps have voted on tile j, then read the four votes at once
+                    const uint32_t q16 = static_cast<uint32_t>(j & 3) << 4;
                     mbar_wait(sb + L::kDec + (q16 >> 1), (j >> 2) & 1);
                     const int tag_keep = (j << 2) | 2;
                     const int4 v4 = lds128_volatile(sb + L::kVotes + q16);
@@ -854,44 +874,23 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     if (G == 1) skip_grp = !keep_any;
                     else skip_grp = !((w >> 1) ? (k2 | k3) : (k0 | k1));
                 }
-                // (a warp with a keeping row goes straight on: skip_grp = false, keep_any = true)
                 if (skip_grp) ++n_skip;                      // a9
-            } else if (kDebug && grp_leader && grp_valid) {  // DENSE: nothing is skipped, every margin is +inf
-                if (a.skip_mask) a.skip_mask[tile_row + j] = 0;
-                if (want_margin) a.margin[tile_row + j] = INFINITY;
-            }
-            prev_skip = kSparse && !keep_any;
-            if (kSparse && !keep_any) continue;              // a7: skipped -- m, l, O untouched
-            if (spec) {
-                // tile j is kept although a speculative S_x(j+1) is being written over S_x: let that MMA finish before
-                // P_x goes into the same columns (the MMA warp issues S_x(j+1) again after P_x V_j)
-                mbar_wait(sb + L::kSFull, sfpar);
-                sfpar ^= 1u;
-                tc_fence_after();
-            }
-
-            uint64_t rs2 = pack_f32x2(0.f, 0.f);             // this tile's row sum, one packed pair of chains
-            if (kSparse && G == 2 && skip_grp) {
-                // this half skipped but its partner half kept: contribute P = 0, statistics untouched
-                uint32_t z[16];
-#pragma unroll
-                for (int i = 0; i < 16; ++i) z[i] = 0u;
-#pragma unroll
-                for (int c = 0; c < BC / 32; ++c) tmem_st_x16(tS + c * 16, z);
-                tmem_wait_st();
-                tc_fence_before();
-                mbar_arrive(sb + L::kPHalf);
-            } else {
-                // ---- online softmax update (a5)
-                if (j == 0) {
-                    m_used = mhat2;
-                    m_gate = mhat2 + kRescaleThreshold;
-                } else {
-                    const bool need = mhat2 > m_gate;
-                    if (__any_sync(0xffffffffu, need)) {
-                        const float alpha = need ? fast_exp2(m_used - mhat2) : 1.f;
-                        if (need) { m_used = mhat2; m_gate = mhat2 + kRescaleThreshold; }
-                        l *= alpha;
+                if (kSparse && !keep_any) {                  // a7: skipped -- m, l, O untouched
+                    prev_skip = true;
+                    continue;
+                }
+                if (spec) {
+                    // tile j is kept although a speculative S_x(j+1) is being written over S_x: let that MMA finish before
+                    // P_x goes into the same columns (the MMA warp issues S_x(j+1) again after P_x V_j)
+                    mbar_wait(sb + L::kSFull, sfpar);
+                    sfpar ^= 1u;
+                    tc_fence_after();
+                }
+                if (need_any && !(kSparse && G == 2 && skip_grp)) {
+                    const float alpha = need ? fast_exp2(m_used - mhat2) : 1.f;
+                    if (need) { m_used = mhat2; m_gate = mhat2 + kRescaleThreshold; }
+                    l *= alpha;
+                    if (j > 0) {
 #pragma unroll
                         for (int c = 0; c < D / 32; ++c) {   // O_r *= alpha (PV of tile j-1 has completed: s_full(j))
                             uint32_t o[32];
@@ -903,6 +902,23 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         }
                     }
                 }
+            }
+            prev_skip = false;
+
+            uint64_t rs2 = pack_f32x2(0.f, 0.f);             // this tile's row sum, one packed pair of chains
+            if (kSparse && G == 2 && skip_grp) {
+                // this half skipped but its partner half kept: contribute P = 0, statistics untouched
+                uint32_t z[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) z[i] = 0u;
+#pragma unroll
+                for (int c = 0; c < BC / 32; ++c) tmem_st_x16(tS + c * 16, z);
+                tmem_wait_st();
+                tc_fence_before();
+#pragma unroll
+                for (int h = 0; h < kHand - 1; ++h) mbar_arrive(sb + L::kPPart + 8 * h);
+            } else {
+                // ---- online softmax update (a5), second part
                 // x = s * scale - m for two logits per FFMA2, row sums as one packed pair per FADD2
                 const float neg_m = -m_used;
                 const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
@@ -912,10 +928,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     uint32_t pk[16];
                     exp_chunk(su[c], scale2, negm2, rs2, pk);
                     tmem_st_x16(tS + c * 16, pk);
-                    if (c == BC / 64 - 1) {                  // first half of P_X is in TMEM: its P V MMAs may start
+                    if ((c + 1) % (BC / 32 / kHand) == 0 && c + 1 < BC / 32) {   // a part of P_X is in TMEM: its P V MMAs may start
                         tmem_wait_st();
                         tc_fence_before();
-                        mbar_arrive(sb + L::kPHalf);
+                        mbar_arrive(sb + L::kPPart + 8 * ((c + 1) / (BC / 32 / kHand) - 1));
                     }
                 }
             }

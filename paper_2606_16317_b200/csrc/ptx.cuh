@@ -22,6 +22,22 @@ __device__ __forceinline__ void fence_mbar_init() {
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Predicated forms for "one lane of the warp signals": a predicate on the instruction instead of a branch around it
+// (a divergent single-lane block costs a BSSY / BRA / BSYNC / WARPSYNC sequence on the softmax warps' critical path).
+__device__ __forceinline__ void mbar_arrive_if(uint32_t bar, bool pred) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.u32 p, %1, 0;\n\t"
+        "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n\t}"
+        ::"r"(bar), "r"(static_cast<uint32_t>(pred)) : "memory");
+}
+__device__ __forceinline__ void st_shared_u32_if(uint32_t saddr, uint32_t val, bool pred) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.u32 p, %2, 0;\n\t"
+        "@p st.volatile.shared.u32 [%0], %1;\n\t}"
+        ::"r"(saddr), "r"(val), "r"(static_cast<uint32_t>(pred)) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }

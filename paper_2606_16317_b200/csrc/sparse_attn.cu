@@ -13,14 +13,11 @@
 #include "fwd_kernel.cuh"
 #include "reorder_kernel.cuh"
 #include "select_kernel.cuh"
+#include "stats_kernel.cuh"
 
 // K / V ring depths of the D = 128 kernels (Q 64 KB + (NK + NV) x 32 KB must fit in 227 KB)
-#ifndef DSA_NK
-#define DSA_NK 3
-#endif
-#ifndef DSA_NV
-#define DSA_NV 2
-#endif
+constexpr int DSA_NK = 3;
+constexpr int DSA_NV = 2;
 
 namespace {
 
@@ -485,6 +482,39 @@ int sparse_attn_reorder_tokens(const void* src, void* dst, int B, int H, int N, 
         dsa::reorder_tokens_kernel<8><<<grid, 256, 0, st>>>(static_cast<const uint4*>(src), static_cast<uint4*>(dst), perm, rows, N, inverse ? 1 : 0);
     CUDA_TRY(cudaGetLastError());
     g_reorder_launches.fetch_add(1);
+    return 0;
+}
+
+int sparse_attn_recall_stats(const float* lse_retained, const float* lse_dense, int64_t n_rows, double* stats_out, void* stream) {
+    g_last_error[0] = '\0';
+    if (!lse_retained || !lse_dense || !stats_out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "lse_retained, lse_dense and stats_out must not be NULL");
+    if (n_rows <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "n_rows must be positive");
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    dsa::stats_init_kernel<<<1, 1, 0, st>>>(stats_out, INFINITY, 0.0);
+    const int grid = static_cast<int>(std::min<int64_t>((n_rows + 255) / 256, 148 * 8));
+    dsa::recall_stats_kernel<<<grid, 256, 0, st>>>(lse_retained, lse_dense, n_rows, stats_out);
+    CUDA_TRY(cudaGetLastError());
+    g_reorder_launches.fetch_add(2);
+    return 0;
+}
+
+int sparse_attn_output_error(const void* out_a, const void* out_b, int64_t n_elems, double* stats_out, void* stream) {
+    g_last_error[0] = '\0';
+    if (!out_a || !out_b || !stats_out) return fail(SPARSE_ATTN_ERR_NULL_POINTER, "out_a, out_b and stats_out must not be NULL");
+    if (n_elems <= 0 || (n_elems & 1)) return fail(SPARSE_ATTN_ERR_SHAPE, "n_elems must be positive and even");
+    if ((reinterpret_cast<uintptr_t>(out_a) | reinterpret_cast<uintptr_t>(out_b)) & 3u)
+        return fail(SPARSE_ATTN_ERR_ALIGNMENT, "out_a and out_b must be 4-byte aligned");
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    dsa::stats_init_kernel<<<1, 1, 0, st>>>(stats_out, 0.0, 0.0);
+    const int64_t n2 = n_elems / 2;
+    const int grid = static_cast<int>(std::min<int64_t>((n2 + 255) / 256, 148 * 8));
+    dsa::output_error_kernel<<<grid, 256, 0, st>>>(static_cast<const __nv_bfloat162*>(out_a), static_cast<const __nv_bfloat162*>(out_b), n2, stats_out);
+    CUDA_TRY(cudaGetLastError());
+    g_reorder_launches.fetch_add(2);
     return 0;
 }
 

@@ -100,7 +100,8 @@ def test_gpu_block_stats_and_greedy_selector(seed):
         else:
             D, tile, B, H = 128, 128, 1, 2
             rng = np.random.default_rng([seed, N, D, 9])
-            qb, kb, vb = (f32_to_bf16_bits(rng.standard_normal((B, H, N, D), dtype=np.float32) * 1.6) for _ in range(3))
+            qb, kb = (f32_to_bf16_bits(rng.standard_normal((B, H, N, D), dtype=np.float32) * 1.6) for _ in range(2))
+            vb = f32_to_bf16_bits(rng.standard_normal((B, H, N, D), dtype=np.float32))     # V ~ N(0,1) as in the configs
         q, k, v = (torch.from_numpy(np.ascontiguousarray(x).view(np.int16)).cuda().view(torch.bfloat16) for x in (qb, kb, vb))
         out = torch.empty_like(q)
         lse = torch.empty((B, H, N), device="cuda", dtype=torch.float32)

@@ -147,15 +147,27 @@ def _sample_qtiles(T, rng, n_random):
     return sorted(set([0, T - 1] + [int(x) for x in rng.choice(np.arange(1, T - 1), size=n_random, replace=False)]))
 
 
+def _assert_plain_build_equals_debug_build(parity, q, k, v, dbg, *, mode, lam, tile):
+    """The instantiation bench.py times (no parity outputs: kDebug = false) against the oracle-checked debug run of the
+    same call: equal tile counts, bit-equal out and lse.  The debug build synchronises the vote with named barriers, the
+    plain build with the dec mbarrier and the speculative re-issue path; decisions and arithmetic order are the same."""
+    plain = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=tile, debug=False)
+    np.testing.assert_array_equal(plain.stats, dbg.stats)
+    np.testing.assert_array_equal(plain.out, dbg.out)
+    np.testing.assert_array_equal(plain.lse, dbg.lse)
+
+
 @pytest.mark.parametrize("name,lam_dyn,lam_fix", [("cfg1", -3.0, -1.0), ("cfg1_aligned", -6.0, -6.0)])
 def test_cfg1_full_size_sampled_tiles(parity, seed, name, lam_dyn, lam_fix):
-    """Config 1 (B=1, H=24, N=32760, D=128) in the launch configuration bench.py times; the oracle checks
-    the first, the last (ragged) and random Q tiles of 3 heads against all 256 K tiles."""
+    """Config 1 (B=1, H=24, N=32760, D=128) at full size.  The debug build (skip_mask_out / margin_out set) is checked
+    against the oracle on the first, the last (ragged) and random Q tiles of 3 heads, all 256 K tiles; the plain build
+    -- the launch configuration bench.py times -- must then reproduce the debug run bit for bit."""
     cfg = CONFIGS[name]
     q, k, v = make_qkv(cfg, seed)
     rng = np.random.default_rng([seed, 1234])
     heads = [0, 11, 23]
-    for mode, lam in [(MODE_DENSE, -math.inf), (MODE_DYNAMIC, lam_dyn), (MODE_FIXED, lam_fix)]:
+    for mode, lam in [(MODE_DENSE, -math.inf), (MODE_DYNAMIC, lam_dyn), (MODE_FIXED, lam_fix),
+                      (MODE_DYNAMIC, oracle.lambda_from_preal(1.5, cfg.tile, cfg.N))]:
         gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=cfg.tile)
         parity.check_stats(gpu, cfg.N, cfg.tile)
         rep = parity.ParityReport()
@@ -164,10 +176,77 @@ def test_cfg1_full_size_sampled_tiles(parity, seed, name, lam_dyn, lam_fix):
             parity.compare_head(gpu, h, q[0, h], k[0, h], v[0, h], tile=cfg.tile, mode=mode, lam=lam, qtiles=qt,
                                 report=rep)
         _assert_ok(rep, f"{name} mode={mode} lambda={lam} sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.4f}")
+        _assert_plain_build_equals_debug_build(parity, q, k, v, gpu, mode=mode, lam=lam, tile=cfg.tile)
+
+
+def test_cfg2_contract_generator_extreme_heads(parity, seed):
+    """Config 2's generator (per-head temperature tau_h in [1, 2.5], field sigma_h in [1, 6]): the heads with the
+    smallest and the largest tau_h (logits up to tau^2 sqrt(D) = 11 and 71: different exponent ranges), sampled Q tiles."""
+    from workloads.generator import head_params
+    cfg = CONFIGS["cfg2"]
+    taus = [head_params(cfg, seed, h)[0] for h in range(cfg.H)]
+    heads = [int(np.argmin(taus)), int(np.argmax(taus))]
+    q, k, v = make_qkv(cfg, seed, heads=heads)
+    rng = np.random.default_rng([seed, 222])
+    T = -(-cfg.N // cfg.tile)
+    for mode, lam in [(MODE_DENSE, -math.inf), (MODE_DYNAMIC, oracle.lambda_from_preal(1.5, cfg.tile, cfg.N)),
+                      (MODE_DYNAMIC, -3.0), (MODE_FIXED, -2.0)]:
+        gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=cfg.tile)
+        parity.check_stats(gpu, cfg.N, cfg.tile)
+        rep = parity.ParityReport()
+        for i in range(2):
+            parity.compare_head(gpu, i, q[0, i], k[0, i], v[0, i], tile=cfg.tile, mode=mode, lam=lam,
+                                qtiles=_sample_qtiles(T, rng, 2), report=rep)
+        _assert_ok(rep, f"cfg2 heads {heads} (tau {taus[heads[0]]:.2f}, {taus[heads[1]]:.2f}) mode={mode} lambda={lam:.3f} "
+                        f"sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.4f}")
+        _assert_plain_build_equals_debug_build(parity, q, k, v, gpu, mode=mode, lam=lam, tile=cfg.tile)
+
+
+def test_cfg3_contract_generator_sampled_tiles(parity, seed):
+    """Config 3 as BASELINE.json states it (N = 75600: 591 tiles, 80-row ragged tail; per-head tau / sigma), three heads,
+    first / ragged-last / four random Q tiles, DYNAMIC at the paper's lambda = -6 and -8 and at the
+    strict map of recall 0.9, FIXED at -6."""
+    cfg = CONFIGS["cfg3"]
+    heads = [0, 19, 39]
+    q, k, v = make_qkv(cfg, seed, heads=heads)
+    rng = np.random.default_rng([seed, 333])
+    T = -(-cfg.N // cfg.tile)
+    assert T == 591 and cfg.N - 590 * 128 == 80
+    for mode, lam in [(MODE_DYNAMIC, -6.0), (MODE_DYNAMIC, -8.0), (MODE_DYNAMIC, oracle.lambda_from_recall(0.9, cfg.N)),
+                      (MODE_FIXED, -6.0)]:
+        gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=cfg.tile)
+        parity.check_stats(gpu, cfg.N, cfg.tile)
+        rep = parity.ParityReport()
+        for i in range(len(heads)):
+            parity.compare_head(gpu, i, q[0, i], k[0, i], v[0, i], tile=cfg.tile, mode=mode, lam=lam,
+                                qtiles=_sample_qtiles(T, rng, 4), report=rep)
+        _assert_ok(rep, f"cfg3 heads {heads} mode={mode} lambda={lam:.3f} sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.4f}")
+        _assert_plain_build_equals_debug_build(parity, q, k, v, gpu, mode=mode, lam=lam, tile=cfg.tile)
+
+
+@pytest.mark.parametrize("noise_a", [0.1, 0.9])
+def test_cfg4_drift_generator_sampled_tiles(parity, seed, noise_a):
+    """Config 4 (drift sweep at the 720p shape): X = (1 - a) field + a noise at the two ends of the sweep."""
+    cfg = CONFIGS["cfg4"]
+    heads = [5, 30]
+    q, k, v = make_qkv(cfg, seed, heads=heads, noise_a=noise_a)
+    rng = np.random.default_rng([seed, 444, int(noise_a * 10)])
+    T = -(-cfg.N // cfg.tile)
+    lam = oracle.lambda_from_preal(1.5, cfg.tile, cfg.N)
+    for mode in (MODE_DYNAMIC, MODE_FIXED):
+        gpu = parity.run_gpu(q, k, v, mode=mode, lam=lam, tile=cfg.tile)
+        parity.check_stats(gpu, cfg.N, cfg.tile)
+        rep = parity.ParityReport()
+        for i in range(len(heads)):
+            parity.compare_head(gpu, i, q[0, i], k[0, i], v[0, i], tile=cfg.tile, mode=mode, lam=lam,
+                                qtiles=_sample_qtiles(T, rng, 2), report=rep)
+        _assert_ok(rep, f"cfg4 a={noise_a} mode={mode} lambda={lam:.3f} sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.4f}")
+        _assert_plain_build_equals_debug_build(parity, q, k, v, gpu, mode=mode, lam=lam, tile=cfg.tile)
 
 
 def test_cfg3_shape_sampled_tiles(parity, seed):
-    """Config 3's N = 75600 (591 tiles: odd tile count, 80-row ragged tail) on 2 heads of the aligned variant."""
+    """Config 3's N = 75600 on 2 heads of the supplementary aligned variant (where most tiles are skipped: long skip runs,
+    the speculative Q K^T path)."""
     cfg = CONFIGS["cfg3_aligned"]
     q, k, v = make_qkv(cfg, seed, heads=[3, 17])
     rng = np.random.default_rng([seed, 4321])
@@ -180,6 +259,7 @@ def test_cfg3_shape_sampled_tiles(parity, seed):
             parity.compare_head(gpu, h, q[0, h], k[0, h], v[0, h], tile=cfg.tile, mode=mode, lam=lam, qtiles=qt,
                                 report=rep)
         _assert_ok(rep, f"cfg3_aligned mode={mode} lambda={lam} sparsity={gpu.stats[:, 1].sum() / gpu.stats.sum():.4f}")
+        _assert_plain_build_equals_debug_build(parity, q, k, v, gpu, mode=mode, lam=lam, tile=cfg.tile)
 
 
 # ------------------------------------------------------------------ invariants that hold at any size

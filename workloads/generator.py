@@ -121,15 +121,29 @@ def make_head(cfg: WorkloadConfig, seed: int, head: int, noise_a: Optional[float
     return f32_to_bf16_bits(q), f32_to_bf16_bits(k), f32_to_bf16_bits(v)
 
 
-def make_qkv(cfg: WorkloadConfig, seed: int, heads=None, noise_a: Optional[float] = None):
-    """Returns (q, k, v) uint16 arrays [B, len(heads), N, D]; B is 1 in every contract config."""
+def _make_head_job(args):
+    return make_head(*args)
+
+
+def make_qkv(cfg: WorkloadConfig, seed: int, heads=None, noise_a: Optional[float] = None, workers: int = 0):
+    """Returns (q, k, v) uint16 arrays [B, len(heads), N, D]; B is 1 in every contract config.
+
+    workers > 1 draws the heads in that many spawned processes (every head has its own substreams, so the bits do not
+    depend on the worker count); `spawn`, not `fork`: the caller may already hold a CUDA context."""
     heads = list(range(cfg.H)) if heads is None else list(heads)
     q = np.empty((cfg.B, len(heads), cfg.N, cfg.D), dtype=np.uint16)
     k = np.empty_like(q)
     v = np.empty_like(q)
-    for b in range(cfg.B):
-        for i, h in enumerate(heads):
-            q[b, i], k[b, i], v[b, i] = make_head(cfg, seed + 7919 * b, h, noise_a)
+    jobs = [(cfg, seed + 7919 * b, h, noise_a) for b in range(cfg.B) for h in heads]
+    if workers > 1 and len(jobs) > 1:
+        import multiprocessing as mp
+        with mp.get_context("spawn").Pool(min(workers, len(jobs))) as pool:
+            results = pool.map(_make_head_job, jobs, chunksize=1)
+    else:
+        results = [make_head(*j) for j in jobs]
+    for n, (hq, hk, hv) in enumerate(results):
+        b, i = divmod(n, len(heads))
+        q[b, i], k[b, i], v[b, i] = hq, hk, hv
     return q, k, v
 
 
