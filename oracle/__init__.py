@@ -18,3 +18,4 @@ from .oracle import (  # noqa: F401
 from .brute_force import brute_force_head  # noqa: F401
 from .reorder import brick_permutation, reorder  # noqa: F401
 from .block_mass import block_mass, block_sqmass, eq3_lhs, select_greedy, select_topk, select_topp  # noqa: F401
+from .analysis import KURTOSIS_BINS, excess_kurtosis, kurtosis_bin, row_probabilities, row_topk_curve, table3  # noqa: F401
