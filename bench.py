@@ -474,19 +474,69 @@ def report_cfg4(args, sa, torch):
     return out
 
 
+def report_masks(args, sa, torch):
+    """SURVEY.md 8(f) NEXT-4 / PAPER.md:196-206 (Fig. 3): block masks of Top-K, Top-P, the section-3 greedy mask, FIXED
+    (BLASST) and DYNAMIC (DynSparse) on synthetic P-matrix regimes, every method's parameter bisected to the same mean row
+    recall; the bitmaps as text ('#' retained, '.' skipped)."""
+    from paper_2606_16317_b200 import analysis
+    from workloads.scenarios import SCENARIOS, make_scenario, scenario_notes
+    notes = scenario_notes()
+    out = {"report": "masks", "shape": "one head, N=4096, D=128, 128x128 tiles (32x32 bitmaps)", "targets": {}}
+    for target in (0.90, 0.95, 0.99):
+        per = {}
+        for name in SCENARIOS:
+            q, k, v = make_scenario(name, args.seed)
+            res = analysis.compare_masks(q, k, v, target)
+            per[name] = {"note": notes[name],
+                         "methods": {m: {**{k_: v_ for k_, v_ in r.items() if k_ != "mask"},
+                                         **({"mask": analysis.mask_picture(r["mask"])} if target == 0.95 else {})}
+                                     for m, r in res.items()}}
+        mean_sp = {m: float(np.mean([per[n]["methods"][m]["sparsity"] for n in SCENARIOS])) for m in analysis.METHODS}
+        out["targets"]["mean_recall_%.2f" % target] = {"scenarios": per, "mean_sparsity_over_scenarios": mean_sp}
+    return out
+
+
+# Table 3's kurtosis bins (PAPER.md:261-273), (lo, hi]
+KURT_EDGES = (-math.inf, 0.0, 1.0, 3.0, 10.0, 30.0, 100.0, 300.0, 1000.0, 3000.0, 10000.0, math.inf)
+
+
+def report_kurtosis(args, sa, torch):
+    """SURVEY.md 8(f) NEXT-4 / PAPER.md:249-275 (Appendix A.1, Fig. 4, Table 3): sampled rows of P from flat to peaked heads,
+    Top-K over a grid of K, MAE against recall by excess-kurtosis bin: MAE at recall 0.8 +- 0.01 and recall at MAE 0.05 +- 0.005."""
+    from paper_2606_16317_b200 import analysis
+    from workloads.scenarios import kurtosis_heads
+    q, k, v, params = kurtosis_heads(args.seed)
+    t0 = time.perf_counter()
+    rows, keep, kurt, recall, mae = analysis.topk_curves(q, k, v, rows_per_head=128, seed=args.seed)
+    secs = time.perf_counter() - t0
+    edges = np.array(KURT_EDGES[1:-1])
+    bins = np.searchsorted(edges, kurt, side="left")          # bin b: edges[b-1] < kurt <= edges[b]
+    table = []
+    for b in range(len(KURT_EDGES) - 1):
+        sel = bins == b
+        rc, me = recall[sel].ravel(), mae[sel].ravel()
+        a = me[np.abs(rc - 0.8) <= 0.01]
+        c = rc[np.abs(me - 0.05) <= 0.005]
+        table.append({"kurtosis_range": [KURT_EDGES[b], KURT_EDGES[b + 1]], "rows": int(sel.sum()),
+                      "mae_at_recall_0.8": {"n": int(a.size), "mean": float(a.mean()) if a.size else None,
+                                            "std": float(a.std()) if a.size else None},
+                      "recall_at_mae_0.05": {"n": int(c.size), "mean": float(c.mean()) if c.size else None,
+                                             "var": float(c.var()) if c.size else None}})
+    heads = [{"head": h, "tau": params[h][0], "aligned": params[h][1],
+              "kurtosis_median": float(np.median(kurt[rows[:, 0] == h]))} for h in range(len(params))]
+    return {"report": "kurtosis", "shape": f"{len(params)} heads, N={q.shape[2]}, D={q.shape[3]}, 128 sampled rows per head",
+            "n_keep_values": int(keep.size), "seconds_row_topk_curve": secs, "heads": heads, "table3": table,
+            "note": "synthetic rows stand in for Wan 2.2-5B's (PAPER.md:253): the trend, not the numbers, is comparable"}
+
+
 def run_report(args):
     import torch
     import paper_2606_16317_b200 as sa
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (B200); there is no CPU fallback")
     torch.cuda.set_device(0)
-    if args.report in ("masks", "kurtosis"):
-        from paper_2606_16317_b200 import analysis
-        fn = analysis.report_masks if args.report == "masks" else analysis.report_kurtosis
-        out = fn(args.seed)
-    else:
-        out = {"cfg2": report_cfg2, "cfg3": report_cfg3, "cfg4": report_cfg4}[args.report](args, sa, torch)
-    print(json.dumps(out), flush=True)
+    fn = {"cfg2": report_cfg2, "cfg3": report_cfg3, "cfg4": report_cfg4, "masks": report_masks, "kurtosis": report_kurtosis}
+    print(json.dumps(fn[args.report](args, sa, torch)), flush=True)
 
 
 # ---------------------------------------------------------------------------------------------- main

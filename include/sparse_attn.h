@@ -226,6 +226,27 @@ int sparse_attn_select_blocks_greedy(const float* mass, const float* sqmass, uin
 int sparse_attn_recall_stats(const float* lse_retained, const float* lse_dense, int64_t n_rows, double* stats_out, void* stream);
 int sparse_attn_output_error(const void* out_a, const void* out_b, int64_t n_elems, double* stats_out, void* stream);
 
+/*
+ * Row-level accuracy-vs-recall analysis of Appendix A.1 ("We sample random rows from the P matrix and
+ * apply Top-K with different K values to ablate the recall rate.  Excess Kurtosis is used to measure the 'tailedness'
+ * of a data distribution"; Fig. 4, Table 3).  For each sampled query row (bh, r), over ALL N keys of head bh:
+ *     p = softmax(softmax_scale * q_r K^T);   kurtosis = m4 / m2^2 - 3 (population moments of the N values of p);
+ *     for each K = keep_counts[i]: Top-K = the keys with p >= the K-th largest p (ties at the K-th value are all retained),
+ *     recall = sum_TopK p,  O' = sum_TopK p v / recall (Eq. 1),  MAE = mean_d |O_d - O'_d|, O = sum p v.
+ *   q, k, v        device, bf16, [B, H, N, D] contiguous, 16-byte aligned
+ *   rows           HOST, int32 [n_rows][2] = (b * H + h, r); n_rows <= 2^20      keep_counts  HOST, int32 [n_keep], 1 <= K <= N
+ *   kurtosis_out   device, fp64 [n_rows] (NaN for a constant row)
+ *   recall_out, mae_out   device, fp64 [n_rows][n_keep]
+ *   softmax_scale  0 means 1/sqrt(D);   stream  cudaStream_t, NULL = default
+ * One CTA per sampled row; logits and exponentials in fp32, sums and moments in fp64; the K-th largest value is found
+ * exactly (bitwise radix select), no sort.  Allocates n_rows * N * 4 bytes of scratch from the stream-ordered pool,
+ * copies rows / keep_counts (synchronising `stream` once), enqueues one kernel and returns.  An offline analysis tool.
+ * Errors: NULL pointers, bad shape, D not in {64, 128}, a row or K out of range, misaligned buffers, no sm_100 device.
+ */
+int sparse_attn_row_topk_curve(const void* q, const void* k, const void* v, int B, int H, int N, int D, float softmax_scale,
+                               const int32_t* rows, int n_rows, const int32_t* keep_counts, int n_keep,
+                               double* kurtosis_out, double* recall_out, double* mae_out, void* stream);
+
 /* Static string for a status code. */
 const char* sparse_attn_status_string(int status);
 

@@ -29,6 +29,7 @@ EXPORTED_SYMBOLS = (
     "sparse_attn_select_blocks_greedy",
     "sparse_attn_recall_stats",
     "sparse_attn_output_error",
+    "sparse_attn_row_topk_curve",
     "sparse_attn_brick_permutation",
     "sparse_attn_reorder_tokens",
     "sparse_attn_select_blocks",
@@ -93,6 +94,9 @@ def _load():
         lib.sparse_attn_recall_stats.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
         lib.sparse_attn_output_error.restype = ctypes.c_int
         lib.sparse_attn_output_error.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p]
+        lib.sparse_attn_row_topk_curve.restype = ctypes.c_int
+        lib.sparse_attn_row_topk_curve.argtypes = [ctypes.c_void_p] * 3 + [ctypes.c_int] * 4 + [ctypes.c_float, ctypes.c_void_p,
+                                                   ctypes.c_int, ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 4
         lib.sparse_attn_select_blocks.restype = ctypes.c_int
         lib.sparse_attn_select_blocks.argtypes = [ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 5 + [
             ctypes.c_double, ctypes.c_void_p]
@@ -250,6 +254,19 @@ def sparse_attn_select_blocks(mass, skip_mask_out, B, H, T_r, T_c, kind, param, 
     """C entry point `sparse_attn_select_blocks` (device buffers): Top-K / Top-P bitmap from a block-mass matrix."""
     rc = _load().sparse_attn_select_blocks(_ptr(mass), _ptr(skip_mask_out), int(B), int(H), int(T_r), int(T_c), int(kind),
                                            float(param), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+def sparse_attn_row_topk_curve(q, k, v, B, H, N, D, rows, keep_counts, kurtosis_out, recall_out, mae_out, softmax_scale=0.0,
+                               stream=None):
+    """C entry point `sparse_attn_row_topk_curve` (Appendix A.1): rows = host int32 [n_rows, 2] (numpy), keep_counts = host
+    int32 [n_keep] (numpy); q, k, v and the three fp64 outputs are device buffers."""
+    n_rows, n_keep = int(rows.shape[0]), int(keep_counts.shape[0])
+    rc = _load().sparse_attn_row_topk_curve(_ptr(q), _ptr(k), _ptr(v), int(B), int(H), int(N), int(D), float(softmax_scale),
+                                            _ptr(rows), n_rows, _ptr(keep_counts), n_keep, _ptr(kurtosis_out),
+                                            _ptr(recall_out), _ptr(mae_out), _ptr(stream))
     if rc != 0:
         raise SparseAttnError(rc, last_error())
     return rc

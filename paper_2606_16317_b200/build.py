@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsparse_attn.so")
 SOURCES = ["sparse_attn.cu"]
-DEPS = ["sparse_attn.cu", "fwd_kernel.cuh", "reorder_kernel.cuh", "select_kernel.cuh", "stats_kernel.cuh", "ptx.cuh", os.path.join("..", "..", "include", "sparse_attn.h")]
+DEPS = ["sparse_attn.cu", "fwd_kernel.cuh", "reorder_kernel.cuh", "rowcurve_kernel.cuh", "select_kernel.cuh", "stats_kernel.cuh", "ptx.cuh", os.path.join("..", "..", "include", "sparse_attn.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-shared", "-Xcompiler", "-fPIC",

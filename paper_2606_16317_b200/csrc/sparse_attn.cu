@@ -12,6 +12,7 @@
 
 #include "fwd_kernel.cuh"
 #include "reorder_kernel.cuh"
+#include "rowcurve_kernel.cuh"
 #include "select_kernel.cuh"
 #include "stats_kernel.cuh"
 
@@ -515,6 +516,54 @@ int sparse_attn_output_error(const void* out_a, const void* out_b, int64_t n_ele
     dsa::output_error_kernel<<<grid, 256, 0, st>>>(static_cast<const __nv_bfloat162*>(out_a), static_cast<const __nv_bfloat162*>(out_b), n2, stats_out);
     CUDA_TRY(cudaGetLastError());
     g_reorder_launches.fetch_add(2);
+    return 0;
+}
+
+int sparse_attn_row_topk_curve(const void* q, const void* k, const void* v, int B, int H, int N, int D, float softmax_scale,
+                               const int32_t* rows, int n_rows, const int32_t* keep_counts, int n_keep,
+                               double* kurtosis_out, double* recall_out, double* mae_out, void* stream) {
+    g_last_error[0] = '\0';
+    if (!q || !k || !v || !rows || !keep_counts || !kurtosis_out || !recall_out || !mae_out)
+        return fail(SPARSE_ATTN_ERR_NULL_POINTER, "q, k, v, rows, keep_counts and the three outputs must not be NULL");
+    if (B <= 0 || H <= 0 || N <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N must be positive (got %d, %d, %d)", B, H, N);
+    if (N > (1 << 24)) return fail(SPARSE_ATTN_ERR_SHAPE, "N = %d exceeds 2^24", N);
+    if (D != 64 && D != 128) return fail(SPARSE_ATTN_ERR_HEAD_DIM, "D = %d not in {64, 128}", D);
+    if (n_rows <= 0 || n_rows > (1 << 20) || n_keep <= 0 || n_keep > 4096)
+        return fail(SPARSE_ATTN_ERR_SHAPE, "n_rows must be in [1, 2^20] and n_keep in [1, 4096] (got %d, %d)", n_rows, n_keep);
+    if (!(softmax_scale >= 0.f) || std::isinf(softmax_scale))
+        return fail(SPARSE_ATTN_ERR_PARAMS, "softmax_scale must be finite and >= 0 (0 = 1/sqrt(D))");
+    for (int i = 0; i < n_rows; ++i)
+        if (rows[2 * i] < 0 || rows[2 * i] >= B * H || rows[2 * i + 1] < 0 || rows[2 * i + 1] >= N)
+            return fail(SPARSE_ATTN_ERR_PARAMS, "rows[%d] = (%d, %d) outside [0, B*H) x [0, N)", i, rows[2 * i], rows[2 * i + 1]);
+    for (int i = 0; i < n_keep; ++i)
+        if (keep_counts[i] < 1 || keep_counts[i] > N)
+            return fail(SPARSE_ATTN_ERR_PARAMS, "keep_counts[%d] = %d outside [1, N]", i, keep_counts[i]);
+    if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(k) | reinterpret_cast<uintptr_t>(v)) & 15u)
+        return fail(SPARSE_ATTN_ERR_ALIGNMENT, "q, k and v must be 16-byte aligned");
+    int rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int32_t *d_rows = nullptr, *d_keep = nullptr;
+    float* scratch = nullptr;
+    CUDA_TRY(cudaMallocAsync(reinterpret_cast<void**>(&d_rows), sizeof(int32_t) * 2 * n_rows, st));
+    CUDA_TRY(cudaMallocAsync(reinterpret_cast<void**>(&d_keep), sizeof(int32_t) * n_keep, st));
+    CUDA_TRY(cudaMallocAsync(reinterpret_cast<void**>(&scratch), sizeof(float) * static_cast<size_t>(n_rows) * N, st));
+    CUDA_TRY(cudaMemcpyAsync(d_rows, rows, sizeof(int32_t) * 2 * n_rows, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(d_keep, keep_counts, sizeof(int32_t) * n_keep, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));                     // rows / keep_counts may be pageable: the caller may reuse them now
+    const float scale = softmax_scale > 0.f ? softmax_scale : 1.0f / std::sqrt(static_cast<float>(D));
+    auto qp = static_cast<const __nv_bfloat16*>(q), kp = static_cast<const __nv_bfloat16*>(k), vp = static_cast<const __nv_bfloat16*>(v);
+    if (D == 128)
+        dsa::row_topk_curve_kernel<128><<<n_rows, dsa::kRowCurveThreads, 0, st>>>(qp, kp, vp, N, scale, d_rows, d_keep, n_keep, scratch,
+                                                                                  kurtosis_out, recall_out, mae_out);
+    else
+        dsa::row_topk_curve_kernel<64><<<n_rows, dsa::kRowCurveThreads, 0, st>>>(qp, kp, vp, N, scale, d_rows, d_keep, n_keep, scratch,
+                                                                                 kurtosis_out, recall_out, mae_out);
+    CUDA_TRY(cudaGetLastError());
+    g_reorder_launches.fetch_add(1);
+    CUDA_TRY(cudaFreeAsync(scratch, st));
+    CUDA_TRY(cudaFreeAsync(d_keep, st));
+    CUDA_TRY(cudaFreeAsync(d_rows, st));
     return 0;
 }
 

@@ -293,3 +293,44 @@ def test_host_buffer_entry_point(parity, seed):
     dev = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=-2.0, tile=cfg.tile)
     np.testing.assert_array_equal(bf16_bits_to_f64(out).reshape(cfg.H, cfg.N, cfg.D), dev.out)
     np.testing.assert_array_equal(stats.reshape(cfg.H, 2), dev.stats)
+
+
+# ------------------------------------------------------------------ in place of compute-sanitizer (profiles/sanitizer_r02.md)
+def test_sanitizer_cases_run_clean():
+    """Every kernel instantiation on small cases (the script written for compute-sanitizer, which this pool does not
+    allow): finite outputs, consistent counts, no CUDA error."""
+    import importlib.util
+    import os
+    spec = importlib.util.spec_from_file_location("sanitizer_cases", os.path.join(os.path.dirname(__file__), "sanitizer_cases.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    mod.main()
+
+
+@pytest.mark.parametrize("tile_k", [0, 32])
+def test_repeated_launches_are_bit_identical(parity, seed, tile_k):
+    """The timed build on a workload with mixed skip / keep decisions (speculative Q K^T, re-issue after a mis-speculated
+    skip, on-demand V, vote ring), 20 launches: a race between the softmax warps, the issuers and the V producer would
+    show up as a run that differs from the others.  The first run is the one the oracle checks."""
+    import torch
+    cfg = CONFIGS["cfg1_aligned"]
+    heads = [0, 7]
+    q, k, v = make_qkv(cfg, seed, heads=heads)
+    lam = oracle.lambda_from_preal(1.5, tile_k or cfg.tile, cfg.N)
+    first = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=lam, tile=cfg.tile, tile_k=tile_k, debug=False)
+    assert 0.2 < first.stats[:, 1].sum() / first.stats.sum() < 0.95
+    T = 256
+    for i, h in enumerate(heads):
+        ref = oracle.run_head(q[0, i], k[0, i], v[0, i], tile=cfg.tile, tile_k=tile_k or cfg.tile, lam=lam, mode=MODE_DYNAMIC,
+                              qtiles=[0, 100, T - 1])
+        o_ref, lse_ref = ref.rows()
+        rows = np.concatenate([np.arange(t * 128, min((t + 1) * 128, cfg.N)) for t in (0, 100, T - 1)])
+        if np.all(np.abs(ref.margin) > parity.MARGIN_TOL):
+            assert np.abs(first.out[i][rows] - o_ref).max() < parity.OUT_MAX_ABS
+            assert np.abs(first.lse[i][rows] - lse_ref).max() < parity.LSE_ABS
+    for _ in range(19):
+        again = parity.run_gpu(q, k, v, mode=MODE_DYNAMIC, lam=lam, tile=cfg.tile, tile_k=tile_k, debug=False)
+        np.testing.assert_array_equal(again.stats, first.stats)
+        np.testing.assert_array_equal(again.out, first.out)
+        np.testing.assert_array_equal(again.lse, first.lse)
+    torch.cuda.synchronize()
