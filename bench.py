@@ -282,6 +282,22 @@ def mode_entry(g, BH_total, ms, per, st_all, st_local):
             "executed_flop_per_launch_rank0": executed_flop(g.B * g.H, cfg.N, cfg.D, st_local)}
 
 
+def pair_stats(mask):
+    """Diagnostic of the two-Q-tiles-per-CTA design: the two slots of a CTA stream the same K / V tiles in
+    lock-step, so a K tile costs the CTA less only when BOTH of its Q tiles skip it.  mask: uint8 [B, H, T_r, T_c], 1 = skip
+    (DYNAMIC mode's own decisions).  Returns the fraction of (CTA, K tile) pairs skipped by both / by exactly one slot and the
+    speed-up bound 1 / (1 - joint / 2) of the lock-step pair (the MMA-bound model of a single Q tile is 1 / (1 - s / 2))."""
+    m = mask.reshape(-1, mask.shape[-2], mask.shape[-1]).astype(bool)
+    T_r = m.shape[1]
+    even, odd = m[:, 0:T_r - (T_r % 2):2], m[:, 1::2]
+    joint, one = float((even & odd).sum()), float((even ^ odd).sum())
+    pairs = float(even.size)
+    if T_r % 2:                                             # the last CTA of a head holds one Q tile
+        joint += float(m[:, -1].sum())
+        pairs += float(m[:, -1].size)
+    return {"both_slots_skip": joint / pairs, "one_slot_skips": one / pairs, "lockstep_model": 1.0 / (1.0 - joint / pairs / 2.0)}
+
+
 def time_reorder(sa, torch, cfg, brick, qkv, scratch_out, steps, warmup):
     """Re-orders q, k, v into brick order with sparse_attn_reorder_tokens and times the four passes a call needs
     (three gathers before the attention, one scatter of `out` after it)."""
@@ -655,6 +671,14 @@ def main():
             if mname != "dense" and "dense" in res:
                 res[mname]["speedup_vs_dense"] = res["dense"]["ms"] / res[mname]["ms"]
                 res[mname]["mma_bound_model"] = 1.0 / (1.0 - res[mname]["sparsity"] / 2.0)
+            if mname == "dynamic" and brick is None:
+                # which skips the pair of Q tiles of a CTA can turn into time (outside the timed region; debug build)
+                T_dec = -(-vcfg.N // vcfg.tile)
+                dmask = torch.zeros((vcfg.B, vcfg.H, T_dec, T_dec), device="cuda", dtype=torch.uint8)
+                g.call(sa.MODE_DYNAMIC, mlam, skip_mask_out=dmask)
+                torch.cuda.synchronize()
+                res[mname]["cta_pair"] = pair_stats(dmask.cpu().numpy())
+                del dmask
         if vi == 1 and brick is None and "dynamic" in res and "dense" in res:
             selectors = selector_comparison(g, res["dynamic"], args.steps, args.warmup)
         if brick is not None and reorder_info is not None:

@@ -100,7 +100,7 @@ struct SmemLayout {
     static constexpr int kSRead = 24;       // the 4 warps of slot X hold S_X(j) in registers          (count 4)
     static constexpr int kPPart = 32;       // p_part[3]: the first 1, 2, 3 parts of P_X written (kept tiles only; count 128)
     static constexpr int kDec = 56;         // dec[4]: the 4 warps of slot X have voted on tile j      (count 4), ring j & 3
-    static constexpr int kVotes = 96;       // votes[4][4]: (j << 2) | vote of warp w on tile j, ring j & 3, 16-B rows
+    static constexpr int kVotes = 96;       // votes[4][4]: vote_word() of warp w on tile j, ring j & 3, 16-B rows
     static constexpr int kWmax = 160;       // wmax[4][4]: per-warp max of t (debug margins), ring j & 3
     static constexpr int kPvMask = 224;     // pvmask[4]: kept sub-tiles of tile j (SUB > 1), ring j & 3
     static constexpr int kPre = 240;        // pre[5][4] (SUB > 1): per-warp sub-tile votes: groups 0, 1 the preliminary
@@ -152,6 +152,23 @@ __device__ __forceinline__ void exp_chunk(const uint32_t (&s)[32], uint64_t scal
     }
 }
 
+// Vote word of warp w of a slot on K tile j (ring j & 3): the tile index as a tag, the per-warp sub-tile bits of the
+// narrow decision tiles (SUB > 1: bit s = "sub-tile s passes the preliminary test", bit SUB + s = "kept for certain"), and
+// the warp's vote on the whole MMA tile: 1 = every row of the warp is below the threshold, 2 = some row is not.
+__device__ __forceinline__ uint32_t vote_word(int j, uint32_t vote, uint32_t sub_bits = 0u) {
+    return (static_cast<uint32_t>(j) << 10) | (sub_bits << 2) | vote;
+}
+__device__ __forceinline__ bool vote_keeps(int word, int j) {          // a keep vote on tile j (and not a stale word)
+    return (static_cast<uint32_t>(word) & ~0x3fcu) == ((static_cast<uint32_t>(j) << 10) | 2u);
+}
+__device__ __forceinline__ bool any_vote_keeps(const int4& v, int j) {
+    return vote_keeps(v.x, j) | vote_keeps(v.y, j) | vote_keeps(v.z, j) | vote_keeps(v.w, j);
+}
+// Speculative Q K^T of the next tile starts once this many tiles in a row were skipped.  A tile retained after a
+// speculated one costs the slot a wasted Q K^T and its re-issue (~ 900 cycles); with scattered skips (the contract
+// generators: 12 % sparsity, runs of length 1) speculating after ONE skipped tile ate everything the skip had saved.
+constexpr int kSpecRun = 2;
+
 // kSparse = false compiles the DENSE mode only (no predicate, no vote, V always fetched);
 // kDebug adds the optional skip_mask_out / margin_out parity outputs.
 // SUB == 0: the block-mass kernel of sparse_attn_block_mass (its own instantiation, so that the forward kernels carry none
@@ -174,7 +191,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     constexpr int kSubD = D / 64;
     // P_X is handed to the issuer in kHand parts of BC / kHand keys, so that the P V steps of a part run while the next
     // part is exponentiated and only the last part's steps follow the last exponential
-    constexpr int kHand = (SUB == 1 && BC / 32 >= 4) ? 4 : 2;
+    constexpr int kHand = (BC / 32 >= 4) ? 4 : 2;
     constexpr uint32_t kIdescQK = umma_idesc_bf16(128, BC, 0);   // S = Q K^T: A, B both K-major
     constexpr uint32_t kIdescPV = umma_idesc_bf16(128, D, 1);    // O += P V: B = V is MN-major (d contiguous)
 
@@ -294,23 +311,29 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 // (barrier dec), fetches V_j if it is needed and not yet there, and after a kept tile fetches V_{j+1}
                 // ahead of its votes (decisions are strongly correlated along j); a wasted prefetch costs L2 traffic
                 // only.  A tile nobody keeps completes its v_full phase with a plain arrive.
+                // The prefetch also survives the first kVPrefetchSkips skipped tiles of a run: where skipped tiles are
+                // scattered among kept ones (the contract generators: 12 % sparsity, short runs) a V_j fetched only after
+                // its votes would expose the L2 latency on every skip -> keep transition; inside long runs nothing is fetched.
+                constexpr int kVPrefetchSkips = 2;
                 load_v(0);                                   // tile 0 is always kept
                 bool have = true;                            // is V_j already in (or on its way to) its slot?
+                int run = 0;                                 // consecutive tiles nobody kept
                 for (int j = 0; j < T_c; ++j) {
                     const int q = j & 3;
-                    const int tag_keep = (j << 2) | 2;
                     const bool has_next = (j + 1) < T_c;
                     bool have_next = false;
+                    if (has_next && have && run < kVPrefetchSkips) { load_v(j + 1); have_next = true; }   // ahead of the votes on j
                     bool keep = false;
                     for (int x = 0; x < nX; ++x) {           // act on the first keep vote, do not wait for both slots
                         mbar_wait(slot(x) + L::kDec + 8 * q, (j >> 2) & 1);
                         const int4 vt = lds128_volatile(slot(x) + L::kVotes + 16 * q);
-                        keep |= (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
+                        keep |= any_vote_keeps(vt, j);
                         if (keep) {
                             if (!have) { load_v(j); have = true; }
                             if (has_next && !have_next) { load_v(j + 1); have_next = true; }
                         }
                     }
+                    run = keep ? 0 : run + 1;
                     if (!have) {                             // nobody keeps tile j: complete its phase without a load
                         wait_slot_free(j);
                         if (lane == 0) mbar_arrive(v_full(j % NV));
@@ -362,7 +385,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             __syncwarp();
             if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
             uint32_t ppar[2] = {0u, 0u};                 // parity of p_half / p_ready: they advance on kept tiles only
-            bool prev_skip[2] = {false, false};          // did slot x skip tile j-1?
+            int skip_run[2] = {0, 0};                    // tiles in a row slot x has skipped, up to tile j-1
             // Sparse modes, speculation: inside a run of skipped tiles the next S_x(j+1) = Q_x K_{j+1}^T is issued as
             // soon as the softmax warps hold S_x(j) in registers (barrier s_read), without waiting for their vote:
             // the vote is then off the critical chain.  If tile j turns out to be kept, the softmax warps let the
@@ -379,7 +402,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 for (int x = 0; x < 2; ++x) {
                     if (x < x_lo || x >= x_hi) continue;
                     const uint32_t sb = slot(x);
-                    const bool spec = kSparse && prev_skip[x] && has_next;
+                    const bool spec = kSparse && skip_run[x] >= kSpecRun && has_next;
                     if (spec) {
                         mbar_wait(sb + L::kSRead, j & 1);
                         tc_fence_after();
@@ -394,10 +417,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         const int q = j & 3;
                         mbar_wait(sb + L::kDec + 8 * q, (j >> 2) & 1);   // all 4 warps of slot x have voted on tile j
                         tc_fence_after();                                // (their votes follow their tcgen05.ld of S_x(j))
-                        const int tag_keep = (j << 2) | 2;
                         const int4 vt = lds128_volatile(sb + L::kVotes + 16 * q);
-                        keep = (vt.x == tag_keep) | (vt.y == tag_keep) | (vt.z == tag_keep) | (vt.w == tag_keep);
-                        prev_skip[x] = !keep;
+                        keep = any_vote_keeps(vt, j);
+                        skip_run[x] = keep ? 0 : skip_run[x] + 1;
                     }
                     if (kGate && nX == 2 && keep) {
                         // two issuers: the P V phases of two slots that both keep their tiles still take turns in the
@@ -505,7 +527,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
         int n_skip = 0;             // decision tiles this (leader) thread saw skipped; executed = all - skipped
         uint32_t sfpar = 0;         // parity of s_full(x): one phase per S_x issued (two for a tile re-issued after a
                                     // mis-speculated skip)
-        bool prev_skip = false;     // did this slot skip tile j-1?
+        int skip_run = 0;           // tiles in a row this slot has skipped, up to tile j-1 (mirrors the issuer's count)
 
         for (int j = 0; j < T_c; ++j) {
             // MASK mode: this tile's byte is fetched before the wait for S_x(j), which hides the global-memory latency
@@ -525,7 +547,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             kst = (kst == k_empty(NK - 1)) ? k_empty(0) : kst + 8;
             tmem_wait_ld();
             // inside a run of skipped tiles the MMA warp issues S_x(j+1) as soon as S_x(j) has left TMEM
-            const bool spec = kSparse && prev_skip && (j + 1) < T_c;
+            const bool spec = kSparse && skip_run >= kSpecRun && (j + 1) < T_c;
             if (kSparse) {                                   // S_x(j) has left TMEM
                 tc_fence_before();
                 mbar_arrive_if(sb + L::kSRead, lane0);
@@ -586,58 +608,36 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 }
                 tc_fence_before();
                 if (lane == 0) {
-                    st_shared_u32(vote_w + 16 * (j & 3), static_cast<uint32_t>((j << 2) | 1));
+                    st_shared_u32(vote_w + 16 * (j & 3), vote_word(j, 1u));
                     mbar_arrive(sb + L::kDec + 8 * (j & 3));
                 }
                 __syncwarp();
-                prev_skip = true;
+                ++skip_run;
                 continue;
             }
-            float mx0 = S_AT(0), mx1 = S_AT(1), mx2 = S_AT(2), mx3 = S_AT(3);   // 4 independent 3-input max chains
+            float mhat2;                                     // tile-local row max (a3), log2 units
+            bool spec_wait = spec;                           // a speculative S_x(j+1) must land before P_x(j) is written
+            if constexpr (SUB <= 1) {
+                float mx0 = S_AT(0), mx1 = S_AT(1), mx2 = S_AT(2), mx3 = S_AT(3);   // 4 independent 3-input max chains
 #pragma unroll
-            for (int c = 4; c + 8 <= BC; c += 8) {
-                mx0 = fmax3(mx0, S_AT(c), S_AT(c + 1));
-                mx1 = fmax3(mx1, S_AT(c + 2), S_AT(c + 3));
-                mx2 = fmax3(mx2, S_AT(c + 4), S_AT(c + 5));
-                mx3 = fmax3(mx3, S_AT(c + 6), S_AT(c + 7));
+                for (int c = 4; c + 8 <= BC; c += 8) {
+                    mx0 = fmax3(mx0, S_AT(c), S_AT(c + 1));
+                    mx1 = fmax3(mx1, S_AT(c + 2), S_AT(c + 3));
+                    mx2 = fmax3(mx2, S_AT(c + 4), S_AT(c + 5));
+                    mx3 = fmax3(mx3, S_AT(c + 6), S_AT(c + 7));
+                }
+                mx0 = fmax3(mx0, S_AT(BC - 4), S_AT(BC - 3));
+                mx1 = fmax3(mx1, S_AT(BC - 2), S_AT(BC - 1));
+                mhat2 = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;
             }
-            mx0 = fmax3(mx0, S_AT(BC - 4), S_AT(BC - 3));
-            mx1 = fmax3(mx1, S_AT(BC - 2), S_AT(BC - 1));
-            const float mhat2 = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * scale_log2;   // tile-local row max (a3)
 
             if constexpr (SUB > 1) {
                 // ============ decision tiles of BC / SUB keys: SUB decisions per MMA tile, in key order
                 constexpr int W = BC / SUB;                  // keys per decision tile (32 or 64)
+                constexpr int CW = W / 32;                   // 32-key chunks (= hand-over parts of P_x) per decision tile
+                constexpr uint32_t kAll = (1u << SUB) - 1u;
                 const int q = j & 3;
-                // the stabiliser m_used follows the max of the WHOLE MMA tile (it only has to bound the exponents; a
-                // sub-tile with a large max is never skipped), so it is fixed before any P of this tile is written
-                if (j == 0) {
-                    m_used = mhat2;
-                } else {
-                    const bool need = mhat2 > m_used + kRescaleThreshold;
-                    if (__any_sync(0xffffffffu, need)) {
-                        const float alpha = need ? fast_exp2(m_used - mhat2) : 1.f;
-                        if (need) m_used = mhat2;
-                        l *= alpha;                          // (m_used + log2 l, hence lse2, is unchanged)
-#pragma unroll
-                        for (int c = 0; c < D / 32; ++c) {   // O_r *= alpha (PV of tile j-1 has completed: s_full(j))
-                            uint32_t o[32];
-                            tmem_ld_x32(tO + c * 32, o);
-                            tmem_wait_ld();
-#pragma unroll
-                            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-                            tmem_st_x32(tO + c * 32, o);
-                        }
-                    }
-                }
-                const float neg_m = -m_used;
-                const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
-                const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
-                // Row maxima of the SUB decision tiles (a3), then a PRELIMINARY test of all of them against the
-                // statistics as they stand before this MMA tile.  Within the tile the reference (LSE, or the running
-                // max) can only grow, so t can only shrink: a sub-tile skipped by the preliminary test is skipped by
-                // the sequential rule too.  One vote round settles every skipped sub-tile (all of them in a run of
-                // skipped tiles); only sub-tiles that pass it AND follow a retained one are tested again.
+                // Row maxima of the SUB decision tiles (a3); the max of the MMA tile is their max
                 float msub[SUB];
 #pragma unroll
                 for (int s = 0; s < SUB; ++s) {
@@ -653,31 +653,94 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     mb = fmax3(mb, S_AT(s * W + W - 2), S_AT(s * W + W - 1));
                     msub[s] = fmaxf(fmaxf(ma, mb), fmaxf(mc, md)) * scale_log2;
                 }
-                uint32_t cand = (1u << SUB) - 1u;            // bit s: sub-tile s passed the preliminary test; bit SUB+s: kept for certain
-                if (!kDebug) {                               // (debug builds test every sub-tile in sequence: margins)
-                    const float ref0 = (mode == kModeDynamic) ? lse2 : m_true;
-                    // Upper bound of how far the reference of this row can grow inside the tile, whatever is retained:
-                    // LSE' <= log2(2^LSE + BC * 2^mhat) (DYNAMIC), m' <= max(m, mhat) (FIXED).  A row whose t stays
-                    // >= lambda even against that bound keeps its sub-tile for certain, with no second vote (bits
-                    // SUB..2 SUB-1).  1e-3 covers the rounding of the approximate ex2 / lg2 in the running statistics.
-                    const float grow_ref = ((mode == kModeDynamic) ? fast_log2(1.f + static_cast<float>(BC) * fast_exp2(mhat2 - ref0))
-                                                                   : fmaxf(0.f, mhat2 - ref0)) + 1e-3f;
-                    uint32_t wc = 0u;
+                mhat2 = msub[0];
 #pragma unroll
-                    for (int s = 0; s < SUB; ++s) {
-                        const bool rs = (j * SUB + s > 0) && (!row_valid || (msub[s] - ref0 < lambda_log2));
-                        if (!__all_sync(0xffffffffu, rs)) wc |= 1u << s;
-                        const bool sure = row_valid && (msub[s] - ref0 - grow_ref >= lambda_log2);
-                        if (__any_sync(0xffffffffu, sure)) wc |= 1u << (SUB + s);
+                for (int s = 1; s < SUB; ++s) mhat2 = fmaxf(mhat2, msub[s]);
+                uint32_t cand = kAll;                        // bit s: sub-tile s passed the preliminary test; bit SUB+s: kept for certain
+                bool all_sure = false;
+                if constexpr (!kDebug) {
+                    // ---- One vote round per MMA tile.  Every warp publishes (a) its vote on the WHOLE tile against the
+                    // statistics as they stand before it (thr = reference + lambda): within the tile the reference (LSE, or
+                    // the running max) can only grow, so t can only shrink, and a sub-tile skipped by this test is skipped by
+                    // the sequential rule too -- if every row of every warp is below thr the MMA tile is skipped, at the cost
+                    // of a tile with one decision; (b) per sub-tile, whether some row passes the test, and whether some row
+                    // keeps the sub-tile FOR CERTAIN: LSE' <= log2(2^LSE + BC 2^mhat) (DYNAMIC), m' <= max(m, mhat) (FIXED)
+                    // bound how far the reference of a row can grow inside the tile, whatever is retained; a row whose max
+                    // stays >= thr even against that bound needs no second vote (1e-3 covers the rounding of the
+                    // approximate ex2 / lg2 in the running statistics).  The votes travel in the vote word the issuer and
+                    // the V warp read anyway (barrier dec); the four warps read all four words.
+                    const bool row_skip_all = mhat2 < thr;   // (rows beyond N: thr = +inf; before the first retained tile: -inf)
+                    const bool wsk = __all_sync(0xffffffffu, row_skip_all);
+                    uint32_t wc = 0u;
+                    if (!wsk) {
+                        const float ref0 = (mode == kModeDynamic) ? lse2 : m_true;
+                        const float grow_ref = ((mode == kModeDynamic) ? fast_log2(1.f + static_cast<float>(BC) * fast_exp2(mhat2 - ref0))
+                                                                       : fmaxf(0.f, mhat2 - ref0)) + 1e-3f;
+#pragma unroll
+                        for (int s = 0; s < SUB; ++s) {
+                            if (!__all_sync(0xffffffffu, msub[s] < thr)) wc |= 1u << s;
+                            const bool sure = (j > 0) && (msub[s] - grow_ref >= thr);
+                            if (__any_sync(0xffffffffu, sure)) wc |= 1u << (SUB + s);
+                        }
                     }
-                    const uint32_t pre = sb + L::kPre + 16 * (j & 1);
-                    if (lane == 0) st_shared_u32(pre + 4 * w, wc);
-                    named_bar_sync(1 + x, 128);
-                    const int4 p4 = lds128_volatile(pre);
-                    cand = static_cast<uint32_t>(p4.x | p4.y | p4.z | p4.w);
+                    tc_fence_before();                       // S_x(j) is in registers: the MMA warp may overwrite it
+                    st_shared_u32_if(vote_w + 16 * q, vote_word(j, wsk ? 1u : 2u, wc), lane0);
+                    mbar_arrive_if(sb + L::kDec + 8 * q, lane0);
+                    mbar_wait(sb + L::kDec + 8 * q, (j >> 2) & 1);
+                    const int4 v4 = lds128_volatile(sb + L::kVotes + 16 * q);
+                    const uint32_t any = static_cast<uint32_t>(v4.x | v4.y | v4.z | v4.w);   // (same tag in all four)
+                    cand = (any >> 2) & 0xffu;
+                    if (!(any & 2u)) {                       // a7: every sub-tile skipped -- m, l, O untouched
+                        n_skip += min(SUB, a.T_c_dec - j * SUB);
+                        ++skip_run;
+                        continue;
+                    }
+                    if (spec) {                              // kept after all: let the speculative S_x(j+1) land first
+                        mbar_wait(sb + L::kSFull, sfpar);
+                        sfpar ^= 1u;
+                        tc_fence_after();
+                        spec_wait = false;
+                    }
+                    all_sure = (cand >> SUB) == kAll;
+                    if (all_sure && w == 0 && lane0) st_shared_u32(sb + L::kPvMask + 4 * q, kAll);
                 }
+                // Every sub-tile retained for certain (the common case wherever little is skipped): the tile takes the very
+                // same straight-line path as a tile with ONE decision (below); otherwise the sub-tile loop.
+                if (!all_sure) {
+                // the stabiliser m_used follows the max of the WHOLE MMA tile (it only has to bound the exponents; a
+                // sub-tile with a large max is never skipped), so it is fixed before any P of this tile is written
+                {
+                    const bool need = mhat2 > m_gate;        // (true for every row at j = 0: m_gate = -inf)
+                    if (__any_sync(0xffffffffu, need)) {
+                        const float alpha = need ? fast_exp2(m_used - mhat2) : 1.f;
+                        if (need) { m_used = mhat2; m_gate = mhat2 + kRescaleThreshold; }
+                        l *= alpha;                          // (m_used + log2 l, hence lse2, is unchanged)
+                        if (j > 0) {
+#pragma unroll
+                            for (int c = 0; c < D / 32; ++c) {   // O_r *= alpha (PV of tile j-1 has completed: s_full(j))
+                                uint32_t o[32];
+                                tmem_ld_x32(tO + c * 32, o);
+                                tmem_wait_ld();
+#pragma unroll
+                                for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+                                tmem_st_x32(tO + c * 32, o);
+                            }
+                        }
+                    }
+                }
+                const float neg_m = -m_used;
+                const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
+                const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
                 uint32_t kept = 0u;                          // bit s: decision sub-tile s retained
-                bool half_sent = false;
+                // P_x is handed to the issuer chunk by chunk (32 keys = one part): a part is final once its chunk of P has
+                // been written, or once its decision tile is known to be skipped (the mask bit stays clear and the issuer
+                // leaves its P V steps out).
+                auto hand_over = [&](int c) {                // (after tmem_wait_st + fence where P was written)
+                    if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
+                    if (c == BC / 32 - 1) mbar_arrive(sb + L::kPReady);
+                    else mbar_arrive(sb + L::kPPart + 8 * c);
+                };
+                int handed = 0;                              // parts handed over so far (in order)
                 // Row sums of retained sub-tiles are folded into l (and LSE) lazily: only a decision that is still open
                 // needs the new LSE (Eq. 6); between sub-tiles that are settled the ex2 streams run back to back.
                 uint64_t acc2 = pack_f32x2(0.f, 0.f);
@@ -701,38 +764,52 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     if (open) fold();                        // this decision is taken with the current statistics
                     const float ref = (mode == kModeDynamic) ? lse2 : m_true;
                     const float t2 = ms - ref;               // Eq. 5, log2 units (+inf before the first retained tile)
-                    const bool row_skip = (jj > 0) && (!row_valid || (t2 < lambda_log2));
+                    const bool row_skip = (jj > 0) && (ms < ref + lam_row);      // (rows beyond N: lam_row = +inf)
                     uint64_t rs2 = pack_f32x2(0.f, 0.f);     // row sum of this sub-tile, two packed chains
-                    auto exp_sub = [&]() {                   // a5 for this sub-tile: P columns and row sum
+                    // a5 for this sub-tile: P columns and row sum; `settled`: the sub-tile is known to be retained, so every
+                    // chunk is handed over as soon as it is in TMEM
+                    auto exp_sub = [&](bool settled) {
 #pragma unroll
-                        for (int c = s * (W / 32); c < (s + 1) * (W / 32); ++c) {
+                        for (int c = s * CW; c < (s + 1) * CW; ++c) {
                             uint32_t pk[16];
                             exp_chunk(su[c], scale2, negm2, rs2, pk);
                             tmem_st_x16(tS + c * 16, pk);
+                            if (settled) {
+                                tmem_wait_st();
+                                tc_fence_before();
+                                hand_over(c);
+                            }
                         }
                     };
                     bool skip_s, did_exp = false;
                     if (!((cand >> s) & 1u)) {
-                        skip_s = true;                       // settled by the preliminary round
+                        skip_s = true;                       // settled by the vote round
                     } else if (!kDebug && (kept == 0u || ((cand >> (SUB + s)) & 1u))) {
                         skip_s = false;                      // statistics unchanged since that round, or kept for certain
                     } else if (kept != 0u) {
-                        // A sub-tile that follows a retained one is exponentiated BEFORE its vote is settled: the
-                        // all-rows vote (shared-memory words + one barrier) then completes in the shadow of the ex2
-                        // work instead of holding it up.  If the vote says skip, the P columns just written are never
-                        // read (mask bit clear) and the row sum is dropped.  Every sub-tile has its own group of vote
-                        // words: a sub-tile in between may be settled without a barrier, so a fast warp can be a whole
-                        // sub-tile ahead of a slow one that is still reading the previous group.
-                        exp_sub();
-                        did_exp = true;
+                        // An open decision after a retained sub-tile (the statistics moved).  A warp that holds a keeping
+                        // row knows the outcome on its own -- one row is enough to retain the sub-tile (R1) -- so it posts
+                        // its vote, counts itself in (bar.arrive) and goes straight on.  A warp whose rows all vote skip
+                        // needs the other three: it exponentiates the sub-tile BEFORE their votes are in, so that the
+                        // exchange completes in the shadow of the ex2 work; if the outcome is skip, the P columns just
+                        // written are never read (mask bit clear) and the row sum is dropped.  Every sub-tile has its own
+                        // vote words and its own barrier: a warp may be a whole sub-tile ahead of another.
                         const bool wv = __all_sync(0xffffffffu, row_skip);
                         const uint32_t sv = sb + L::kPre + 16 * (1 + s);
                         if (lane == 0) st_shared_u32(sv + 4 * w, wv ? 1u : 0u);
-                        named_bar_sync(1 + x, 128);
-                        const int4 v4 = lds128_volatile(sv);
-                        skip_s = (v4.x & v4.y & v4.z & v4.w) != 0;   // all 128 rows of the Q tile (R1)
+                        const uint32_t bar_id = 3u + 3u * x + (s - 1);
+                        if (!wv && !kDebug) {
+                            named_bar_arrive(bar_id, 128);
+                            skip_s = false;
+                        } else {
+                            exp_sub(false);
+                            did_exp = true;
+                            named_bar_sync(bar_id, 128);
+                            const int4 v4 = lds128_volatile(sv);
+                            skip_s = (v4.x & v4.y & v4.z & v4.w) != 0;   // all 128 rows of the Q tile (R1)
+                        }
                     } else {
-                        skip_s = named_bar_red_and(1 + x, 128, row_skip);
+                        skip_s = named_bar_red_and(1 + x, 128, row_skip);   // (debug builds, nothing retained yet)
                     }
                     if (kDebug) {
                         float gm = INFINITY;
@@ -755,14 +832,21 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         }
                     }
                     if (skip_s) {
-                        ++n_skip;
-                        continue;                            // a7: this decision tile leaves m, l, O untouched
+                        ++n_skip;                            // a7: this decision tile leaves m, l, O untouched
+                        if (!kDebug || kept != 0u) {         // the MMA tile is retained: its parts go to the issuer, masked out
+                            tc_fence_before();               // (debug builds: parts ahead of the first retained sub-tile wait)
+#pragma unroll
+                            for (int c = s * CW; c < (s + 1) * CW; ++c) hand_over(c);
+                            handed = (s + 1) * CW;
+                        }
+                        continue;
                     }
-                    if (kept == 0u) {
-                        // first retained sub-tile: the MMA tile is kept -- tell the issuer and the V warp now
+                    if (kDebug && kept == 0u) {
+                        // debug builds take no vote on the whole tile: the first retained sub-tile tells the issuer and the
+                        // V warp that the MMA tile is kept
                         tc_fence_before();
                         if (lane == 0) {
-                            st_shared_u32(vote_w + 16 * q, static_cast<uint32_t>((j << 2) | 2));
+                            st_shared_u32(vote_w + 16 * q, vote_word(j, 2u));
                             mbar_arrive(sb + L::kDec + 8 * q);
                         }
                         __syncwarp();
@@ -771,51 +855,52 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             sfpar ^= 1u;
                             tc_fence_after();
                         }
+                        for (int c = handed; c < s * CW; ++c) hand_over(c);   // the skipped sub-tiles ahead of it (mask bits clear)
                     }
                     kept |= 1u << s;
                     m_true = fmaxf(m_true, ms);
-                    if (!did_exp) exp_sub();
-                    acc2 = add_f32x2(acc2, rs2);
-                    dirty = true;
-                    if (s == SUB / 2 - 1) {
-                        // the first half of the keys is done and something in it was retained: hand it over now, so
-                        // that its P V steps run while the second half is decided and exponentiated
-                        if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
+                    if (!did_exp) {
+                        exp_sub(true);
+                    } else {
                         tmem_wait_st();
                         tc_fence_before();
-                        mbar_arrive(sb + L::kPPart);
-                        half_sent = true;
+#pragma unroll
+                        for (int c = s * CW; c < (s + 1) * CW; ++c) hand_over(c);
                     }
+                    handed = (s + 1) * CW;
+                    acc2 = add_f32x2(acc2, rs2);
+                    dirty = true;
                 }
-                prev_skip = kept == 0u;
-                if (kept == 0u) {                            // every sub-tile skipped: the MMA tile is skipped
+                if (kDebug && kept == 0u) {                  // (debug builds) every sub-tile skipped: the MMA tile is skipped
                     tc_fence_before();
                     if (lane == 0) {
-                        st_shared_u32(vote_w + 16 * q, static_cast<uint32_t>((j << 2) | 1));
+                        st_shared_u32(vote_w + 16 * q, vote_word(j, 1u));
                         mbar_arrive(sb + L::kDec + 8 * q);
                     }
                     __syncwarp();
+                    ++skip_run;
                     continue;
                 }
-                if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
-                tmem_wait_st();
-                tc_fence_before();
-                if (!half_sent) mbar_arrive(sb + L::kPPart); // (release: the mask above is visible to the issuer)
-                mbar_arrive(sb + L::kPReady);
+                // (plain builds: a tile whose every sub-tile was skipped by the sequential rule after the vote round had
+                // kept it goes to the issuer with an empty mask: no P V step is issued)
+                skip_run = 0;
+                for (int c = handed; c < BC / 32; ++c) hand_over(c);   // (ragged tail: parts beyond the last decision tile)
                 fold();                                      // statistics for the next tile, behind the hand-over
+                thr = ((mode == kModeDynamic) ? lse2 : m_true) + lam_row;
                 continue;
+                }   // !all_sure
             }
             // ---- predicate and all-rows vote (a4)
             bool skip_grp = false, keep_any = true, wskip = false;
-            if (kSparse) {
-                // votes[j & 3][w] = (j << 2) | (1: every row of warp w is below the threshold, 2: some row is not).
+            if (kSparse && SUB == 1) {                       // (SUB > 1: voted above, every sub-tile kept for certain)
+                // votes[j & 3][w] = vote_word(j, 1: every row of warp w is below the threshold, 2: some row is not).
                 // The MMA warp combines the four votes itself (barrier dec, one arrival per warp), so an all-skip
                 // decision reaches the tensor pipe without the four warps first synchronising with each other.
                 const bool row_skip = mhat2 < thr;           // Eq. 5 against this row's threshold (false at j = 0)
                 wskip = __all_sync(0xffffffffu, row_skip);
                 const uint32_t q16 = static_cast<uint32_t>(j & 3) << 4;
                 tc_fence_before();                           // S_x(j) is in registers: the MMA warp may overwrite it
-                st_shared_u32_if(vote_w + q16, static_cast<uint32_t>((j << 2) | (wskip ? 1 : 2)), lane0);
+                st_shared_u32_if(vote_w + q16, vote_word(j, wskip ? 1u : 2u), lane0);
                 mbar_arrive_if(sb + L::kDec + (q16 >> 1), lane0);
                 if (kDebug) {
                     float grp_margin = INFINITY;
@@ -861,25 +946,24 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             // tile 0), which spares a j == 0 test.
             const bool need = mhat2 > m_gate;
             const bool need_any = __any_sync(0xffffffffu, need);
-            if (__builtin_expect(wskip || spec || need_any || (kSparse && kDebug), 0)) {
+            if (__builtin_expect(wskip || spec_wait || need_any || (kSparse && kDebug), 0)) {
                 if (wskip) {
                     // every row of this warp is below the threshold: wait (hardware-suspended, no shared-memory
                     // polling) until all four warps have voted on tile j, then read the four votes at once
                     const uint32_t q16 = static_cast<uint32_t>(j & 3) << 4;
                     mbar_wait(sb + L::kDec + (q16 >> 1), (j >> 2) & 1);
-                    const int tag_keep = (j << 2) | 2;
                     const int4 v4 = lds128_volatile(sb + L::kVotes + q16);
-                    const bool k0 = v4.x == tag_keep, k1 = v4.y == tag_keep, k2 = v4.z == tag_keep, k3 = v4.w == tag_keep;
+                    const bool k0 = vote_keeps(v4.x, j), k1 = vote_keeps(v4.y, j), k2 = vote_keeps(v4.z, j), k3 = vote_keeps(v4.w, j);
                     keep_any = k0 | k1 | k2 | k3;
                     if (G == 1) skip_grp = !keep_any;
                     else skip_grp = !((w >> 1) ? (k2 | k3) : (k0 | k1));
                 }
                 if (skip_grp) ++n_skip;                      // a9
                 if (kSparse && !keep_any) {                  // a7: skipped -- m, l, O untouched
-                    prev_skip = true;
+                    ++skip_run;
                     continue;
                 }
-                if (spec) {
+                if (spec_wait) {
                     // tile j is kept although a speculative S_x(j+1) is being written over S_x: let that MMA finish before
                     // P_x goes into the same columns (the MMA warp issues S_x(j+1) again after P_x V_j)
                     mbar_wait(sb + L::kSFull, sfpar);
@@ -903,7 +987,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                     }
                 }
             }
-            prev_skip = false;
+            skip_run = 0;
 
             uint64_t rs2 = pack_f32x2(0.f, 0.f);             // this tile's row sum, one packed pair of chains
             if (kSparse && G == 2 && skip_grp) {

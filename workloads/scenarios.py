@@ -71,9 +71,9 @@ def make_scenario(name: str, seed: int):
 
 
 # Appendix A.1: heads of the 480p shape (N = 32760) from flat to very peaked rows: (tau, aligned)
-KURTOSIS_HEADS: Tuple[Tuple[float, bool], ...] = ((0.5, False), (1.0, False), (1.5, False), (2.5, False),
-                                                  (1.0, True), (1.5, True), (2.0, True), (2.5, True),
-                                                  (3.0, True), (3.5, True), (4.0, True), (5.0, True))
+KURTOSIS_HEADS: Tuple[Tuple[float, bool], ...] = ((0.35, False), (0.5, False), (0.75, False), (1.0, False),
+                                                  (1.25, False), (1.5, False), (2.0, False), (2.5, False),
+                                                  (1.0, True), (1.5, True), (2.0, True), (3.0, True))
 
 
 def kurtosis_heads(seed: int, grid=None, heads=None):
