@@ -635,8 +635,9 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 // ============ decision tiles of BC / SUB keys: SUB decisions per MMA tile, in key order
                 constexpr int W = BC / SUB;                  // keys per decision tile (32 or 64)
                 constexpr int CW = W / 32;                   // 32-key chunks (= hand-over parts of P_x) per decision tile
-                constexpr uint32_t kAll = (1u << SUB) - 1u;
                 const int q = j & 3;
+                const int n_sub = min(SUB, a.T_c_dec - j * SUB);            // decision tiles of this MMA tile (ragged tail: fewer)
+                const uint32_t valid = (1u << n_sub) - 1u;
                 // Row maxima of the SUB decision tiles (a3); the max of the MMA tile is their max
                 float msub[SUB];
 #pragma unroll
@@ -656,60 +657,50 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 mhat2 = msub[0];
 #pragma unroll
                 for (int s = 1; s < SUB; ++s) mhat2 = fmaxf(mhat2, msub[s]);
-                uint32_t cand = kAll;                        // bit s: sub-tile s passed the preliminary test; bit SUB+s: kept for certain
-                bool all_sure = false;
-                if constexpr (!kDebug) {
-                    // ---- One vote round per MMA tile.  Every warp publishes (a) its vote on the WHOLE tile against the
-                    // statistics as they stand before it (thr = reference + lambda): within the tile the reference (LSE, or
-                    // the running max) can only grow, so t can only shrink, and a sub-tile skipped by this test is skipped by
-                    // the sequential rule too -- if every row of every warp is below thr the MMA tile is skipped, at the cost
-                    // of a tile with one decision; (b) per sub-tile, whether some row passes the test, and whether some row
-                    // keeps the sub-tile FOR CERTAIN: LSE' <= log2(2^LSE + BC 2^mhat) (DYNAMIC), m' <= max(m, mhat) (FIXED)
-                    // bound how far the reference of a row can grow inside the tile, whatever is retained; a row whose max
-                    // stays >= thr even against that bound needs no second vote (1e-3 covers the rounding of the
-                    // approximate ex2 / lg2 in the running statistics).  The votes travel in the vote word the issuer and
-                    // the V warp read anyway (barrier dec); the four warps read all four words.
-                    const bool row_skip_all = mhat2 < thr;   // (rows beyond N: thr = +inf; before the first retained tile: -inf)
-                    const bool wsk = __all_sync(0xffffffffu, row_skip_all);
-                    uint32_t wc = 0u;
-                    if (!wsk) {
-                        const float ref0 = (mode == kModeDynamic) ? lse2 : m_true;
-                        const float grow_ref = ((mode == kModeDynamic) ? fast_log2(1.f + static_cast<float>(BC) * fast_exp2(mhat2 - ref0))
-                                                                       : fmaxf(0.f, mhat2 - ref0)) + 1e-3f;
+                const float ref0 = (mode == kModeDynamic) ? lse2 : m_true;   // the reference before this MMA tile
+                // ---- Vote round 1 (every MMA tile).  Every warp publishes (a) its vote on the WHOLE tile against the
+                // statistics as they stand before it (thr = reference + lambda): within the tile the reference (LSE, or the
+                // running max) can only grow, so t can only shrink, and a sub-tile skipped by this test is skipped by the
+                // sequential rule too -- if every row of every warp is below thr the MMA tile is skipped, at the cost of a
+                // tile with one decision; (b) per sub-tile, whether some row passes that test (candidates), and whether
+                // some row keeps the sub-tile FOR CERTAIN: LSE' <= log2(2^LSE + BC 2^mhat) (DYNAMIC), m' <= max(m, mhat)
+                // (FIXED) bound how far the reference of a row can grow inside the tile, whatever is retained; a row whose
+                // max stays >= thr even against that bound settles its sub-tile (1e-3 covers the rounding of the
+                // approximate ex2 / lg2 in the running statistics).  The votes travel in the vote word the issuer and the
+                // V warp read anyway (barrier dec); the four warps read all four words.
+                const bool row_skip_all = mhat2 < thr;       // (rows beyond N: thr = +inf; before the first retained tile: -inf)
+                const bool wsk = __all_sync(0xffffffffu, row_skip_all);
+                uint32_t wc = 0u;
+                if (!wsk) {
+                    const float grow_ref = ((mode == kModeDynamic) ? fast_log2(1.f + static_cast<float>(BC) * fast_exp2(mhat2 - ref0))
+                                                                   : fmaxf(0.f, mhat2 - ref0)) + 1e-3f;
 #pragma unroll
-                        for (int s = 0; s < SUB; ++s) {
-                            if (!__all_sync(0xffffffffu, msub[s] < thr)) wc |= 1u << s;
-                            const bool sure = (j > 0) && (msub[s] - grow_ref >= thr);
-                            if (__any_sync(0xffffffffu, sure)) wc |= 1u << (SUB + s);
-                        }
+                    for (int s = 0; s < SUB; ++s) {
+                        if (!__all_sync(0xffffffffu, msub[s] < thr)) wc |= 1u << s;
+                        const bool sure = (j > 0) && (msub[s] - grow_ref >= thr);
+                        if (__any_sync(0xffffffffu, sure)) wc |= 1u << (SUB + s);
                     }
-                    tc_fence_before();                       // S_x(j) is in registers: the MMA warp may overwrite it
-                    st_shared_u32_if(vote_w + 16 * q, vote_word(j, wsk ? 1u : 2u, wc), lane0);
-                    mbar_arrive_if(sb + L::kDec + 8 * q, lane0);
-                    mbar_wait(sb + L::kDec + 8 * q, (j >> 2) & 1);
-                    const int4 v4 = lds128_volatile(sb + L::kVotes + 16 * q);
-                    const uint32_t any = static_cast<uint32_t>(v4.x | v4.y | v4.z | v4.w);   // (same tag in all four)
-                    cand = (any >> 2) & 0xffu;
-                    if (!(any & 2u)) {                       // a7: every sub-tile skipped -- m, l, O untouched
-                        n_skip += min(SUB, a.T_c_dec - j * SUB);
-                        ++skip_run;
-                        continue;
-                    }
+                }
+                tc_fence_before();                           // S_x(j) is in registers: the MMA warp may overwrite it
+                st_shared_u32_if(vote_w + 16 * q, vote_word(j, wsk ? 1u : 2u, wc), lane0);
+                mbar_arrive_if(sb + L::kDec + 8 * q, lane0);
+                mbar_wait(sb + L::kDec + 8 * q, (j >> 2) & 1);
+                const int4 v4 = lds128_volatile(sb + L::kVotes + 16 * q);
+                const uint32_t any = static_cast<uint32_t>(v4.x | v4.y | v4.z | v4.w);   // (same tag in all four)
+                const bool tile_kept = (any & 2u) != 0u;
+                const uint32_t cand = (any >> 2) & valid;    // bit s: sub-tile s passed the test of round 1
+                uint32_t kept = 0u;                          // bit s: decision sub-tile s retained
+                float rsum[SUB];                             // row sums of the exponentiated sub-tiles
+#pragma unroll
+                for (int s = 0; s < SUB; ++s) rsum[s] = 0.f;
+                if (tile_kept) {
                     if (spec) {                              // kept after all: let the speculative S_x(j+1) land first
                         mbar_wait(sb + L::kSFull, sfpar);
                         sfpar ^= 1u;
                         tc_fence_after();
-                        spec_wait = false;
                     }
-                    all_sure = (cand >> SUB) == kAll;
-                    if (all_sure && w == 0 && lane0) st_shared_u32(sb + L::kPvMask + 4 * q, kAll);
-                }
-                // Every sub-tile retained for certain (the common case wherever little is skipped): the tile takes the very
-                // same straight-line path as a tile with ONE decision (below); otherwise the sub-tile loop.
-                if (!all_sure) {
-                // the stabiliser m_used follows the max of the WHOLE MMA tile (it only has to bound the exponents; a
-                // sub-tile with a large max is never skipped), so it is fixed before any P of this tile is written
-                {
+                    // the stabiliser m_used follows the max of the WHOLE MMA tile (it only has to bound the exponents; a
+                    // sub-tile with a large max is never skipped), so it is fixed before any P of this tile is written
                     const bool need = mhat2 > m_gate;        // (true for every row at j = 0: m_gate = -inf)
                     if (__any_sync(0xffffffffu, need)) {
                         const float alpha = need ? fast_exp2(m_used - mhat2) : 1.f;
@@ -727,94 +718,120 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             }
                         }
                     }
-                }
-                const float neg_m = -m_used;
-                const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
-                const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
-                uint32_t kept = 0u;                          // bit s: decision sub-tile s retained
-                // P_x is handed to the issuer chunk by chunk (32 keys = one part): a part is final once its chunk of P has
-                // been written, or once its decision tile is known to be skipped (the mask bit stays clear and the issuer
-                // leaves its P V steps out).
-                auto hand_over = [&](int c) {                // (after tmem_wait_st + fence where P was written)
-                    if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
-                    if (c == BC / 32 - 1) mbar_arrive(sb + L::kPReady);
-                    else mbar_arrive(sb + L::kPPart + 8 * c);
-                };
-                int handed = 0;                              // parts handed over so far (in order)
-                // Row sums of retained sub-tiles are folded into l (and LSE) lazily: only a decision that is still open
-                // needs the new LSE (Eq. 6); between sub-tiles that are settled the ex2 streams run back to back.
-                uint64_t acc2 = pack_f32x2(0.f, 0.f);
-                bool dirty = false;
-                auto fold = [&]() {
-                    if (dirty) {
-                        float r0, r1;
-                        unpack_f32x2(acc2, r0, r1);
-                        l += r0 + r1;
-                        if (mode == kModeDynamic) lse2 = m_used + fast_log2(l);
-                        acc2 = pack_f32x2(0.f, 0.f);
-                        dirty = false;
+                    const float neg_m = -m_used;
+                    const uint64_t scale2 = pack_f32x2(scale_log2, scale_log2);
+                    const uint64_t negm2 = pack_f32x2(neg_m, neg_m);
+                    // Settled after round 1: the FIRST candidate is retained (nothing was retained before it in this tile,
+                    // so its test of round 1 stands), and so is every candidate some row keeps for certain.  The other
+                    // candidates are OPEN: their outcome depends on which earlier sub-tiles are retained (Eq. 6).
+                    const uint32_t known = ((any >> (2 + SUB)) & cand) | (cand & (0u - cand));
+                    const uint32_t open = cand & ~known;
+                    kept = known;
+                    // P_x goes to the issuer chunk by chunk (32 keys = one part), with the mask of retained sub-tiles
+                    // (a clear bit: the issuer leaves that part's P V steps out).  Parts of settled sub-tiles go at once,
+                    // parts of open ones after round 2.
+                    auto hand_over = [&](int c) {            // (after tmem_wait_st + fence where P was written)
+                        if (w == 0 && lane == 0) st_shared_u32(sb + L::kPvMask + 4 * q, kept);
+                        if (c == BC / 32 - 1) mbar_arrive(sb + L::kPReady);
+                        else mbar_arrive(sb + L::kPPart + 8 * c);
+                    };
+                    // the reference of a row once the sub-tiles of set h (all before s) are retained: LSE(h) = m + log2(l +
+                    // sum_{i in h} rsum_i), summed in key order exactly as the statistics are updated below (Eq. 6);
+                    // FIXED: max(m, max_{i in h} msub_i)
+                    auto ref_after = [&](int s, uint32_t h) {
+                        if (mode == kModeDynamic) {
+                            float lh = l;
+#pragma unroll
+                            for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) lh += rsum[i];
+                            return m_used + fast_log2(lh);
+                        }
+                        float ref = m_true;
+#pragma unroll
+                        for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) ref = fmaxf(ref, msub[i]);
+                        return ref;
+                    };
+                    // a5 for every candidate: all of them are exponentiated in one straight pass -- an open sub-tile that
+                    // round 2 skips has cost its ex2 work and nothing else (its P columns are never read)
+#pragma unroll
+                    for (int s = 0; s < SUB; ++s) {
+                        const bool is_cand = (cand >> s) & 1u, is_known = (known >> s) & 1u;
+                        if (is_cand) {
+                            uint64_t rs2 = pack_f32x2(0.f, 0.f);
+#pragma unroll
+                            for (int c = s * CW; c < (s + 1) * CW; ++c) {
+                                uint32_t pk[16];
+                                exp_chunk(su[c], scale2, negm2, rs2, pk);
+                                tmem_st_x16(tS + c * 16, pk);
+                                if (is_known) {
+                                    tmem_wait_st();
+                                    tc_fence_before();
+                                    hand_over(c);
+                                }
+                            }
+                            float r0, r1;
+                            unpack_f32x2(rs2, r0, r1);
+                            rsum[s] = r0 + r1;
+                        } else {                             // skipped in round 1 (or beyond the last key): masked out
+#pragma unroll
+                            for (int c = s * CW; c < (s + 1) * CW; ++c) hand_over(c);
+                        }
                     }
-                };
+                    if (open != 0u) {
+                        // ---- Vote round 2 (only where something is open): every row evaluates the rule for each open
+                        // sub-tile s under every set h of retained earlier sub-tiles that is still possible, and the warps
+                        // exchange the "all my rows vote skip" bits of all of them at once; the sequential rule is then
+                        // resolved from the exchanged bits along the sets that actually materialise, identically in every
+                        // warp: one exchange instead of one per sub-tile.
+                        uint32_t bits = 0u;                  // bit (2^s - 2 + h), h a subset of {0 .. s-1}
 #pragma unroll
-                for (int s = 0; s < SUB; ++s) {
-                    const int jj = j * SUB + s;              // decision tile index along the keys
-                    if (jj >= a.T_c_dec) break;              // beyond the last key (ragged tail): no such tile
-                    const float ms = msub[s];
-                    const bool open = ((cand >> s) & 1u) && (kDebug || (kept != 0u && !((cand >> (SUB + s)) & 1u)));
-                    if (open) fold();                        // this decision is taken with the current statistics
-                    const float ref = (mode == kModeDynamic) ? lse2 : m_true;
-                    const float t2 = ms - ref;               // Eq. 5, log2 units (+inf before the first retained tile)
-                    const bool row_skip = (jj > 0) && (ms < ref + lam_row);      // (rows beyond N: lam_row = +inf)
-                    uint64_t rs2 = pack_f32x2(0.f, 0.f);     // row sum of this sub-tile, two packed chains
-                    // a5 for this sub-tile: P columns and row sum; `settled`: the sub-tile is known to be retained, so every
-                    // chunk is handed over as soon as it is in TMEM
-                    auto exp_sub = [&](bool settled) {
+                        for (int s = 1; s < SUB; ++s) {
 #pragma unroll
-                        for (int c = s * CW; c < (s + 1) * CW; ++c) {
-                            uint32_t pk[16];
-                            exp_chunk(su[c], scale2, negm2, rs2, pk);
-                            tmem_st_x16(tS + c * 16, pk);
-                            if (settled) {
-                                tmem_wait_st();
-                                tc_fence_before();
-                                hand_over(c);
+                            for (int h = 0; h < (1 << s); ++h) {
+                                const uint32_t below = (1u << s) - 1u;
+                                // possible: h retains every settled earlier sub-tile and nothing round 1 skipped
+                                const bool possible = ((open >> s) & 1u) && ((h & ~cand) == 0u) && ((h & known & below) == (known & below));
+                                if (possible) {              // (uniform over the four warps)
+                                    const bool rskip = msub[s] < ref_after(s, h) + lam_row;   // (rows beyond N: lam_row = +inf)
+                                    if (__all_sync(0xffffffffu, rskip)) bits |= 1u << ((1 << s) - 2 + h);
+                                }
                             }
                         }
-                    };
-                    bool skip_s, did_exp = false;
-                    if (!((cand >> s) & 1u)) {
-                        skip_s = true;                       // settled by the vote round
-                    } else if (!kDebug && (kept == 0u || ((cand >> (SUB + s)) & 1u))) {
-                        skip_s = false;                      // statistics unchanged since that round, or kept for certain
-                    } else if (kept != 0u) {
-                        // An open decision after a retained sub-tile (the statistics moved).  A warp that holds a keeping
-                        // row knows the outcome on its own -- one row is enough to retain the sub-tile (R1) -- so it posts
-                        // its vote, counts itself in (bar.arrive) and goes straight on.  A warp whose rows all vote skip
-                        // needs the other three: it exponentiates the sub-tile BEFORE their votes are in, so that the
-                        // exchange completes in the shadow of the ex2 work; if the outcome is skip, the P columns just
-                        // written are never read (mask bit clear) and the row sum is dropped.  Every sub-tile has its own
-                        // vote words and its own barrier: a warp may be a whole sub-tile ahead of another.
-                        const bool wv = __all_sync(0xffffffffu, row_skip);
-                        const uint32_t sv = sb + L::kPre + 16 * (1 + s);
-                        if (lane == 0) st_shared_u32(sv + 4 * w, wv ? 1u : 0u);
-                        const uint32_t bar_id = 3u + 3u * x + (s - 1);
-                        if (!wv && !kDebug) {
-                            named_bar_arrive(bar_id, 128);
-                            skip_s = false;
-                        } else {
-                            exp_sub(false);
-                            did_exp = true;
-                            named_bar_sync(bar_id, 128);
-                            const int4 v4 = lds128_volatile(sv);
-                            skip_s = (v4.x & v4.y & v4.z & v4.w) != 0;   // all 128 rows of the Q tile (R1)
+                        const uint32_t ex = sb + L::kPre + 16 * (j & 1);
+                        if (lane == 0) st_shared_u32(ex + 4 * w, bits);
+                        named_bar_sync(1 + x, 128);
+                        const int4 b4 = lds128_volatile(ex);
+                        const uint32_t allskip = static_cast<uint32_t>(b4.x & b4.y & b4.z & b4.w);   // all 128 rows (R1)
+#pragma unroll
+                        for (int s = 1; s < SUB; ++s) {
+                            if ((open >> s) & 1u) {
+                                const uint32_t h = kept & ((1u << s) - 1u);          // what was actually retained before s
+                                if (!((allskip >> ((1 << s) - 2 + h)) & 1u)) kept |= 1u << s;
+                            }
                         }
-                    } else {
-                        skip_s = named_bar_red_and(1 + x, 128, row_skip);   // (debug builds, nothing retained yet)
+                        tmem_wait_st();
+                        tc_fence_before();
+#pragma unroll
+                        for (int s = 1; s < SUB; ++s) {
+                            if ((open >> s) & 1u) {
+#pragma unroll
+                                for (int c = s * CW; c < (s + 1) * CW; ++c) hand_over(c);
+                            }
+                        }
                     }
-                    if (kDebug) {
+                }
+                if (kDebug) {
+                    // parity outputs: the decision of every sub-tile and its margin g = max_r t_r - lambda, t evaluated against
+                    // the reference the sequential rule saw (the retained sub-tiles before it)
+                    float lrun = l, mrun = m_true;
+                    bool moved = false;
+#pragma unroll
+                    for (int s = 0; s < SUB; ++s) {
+                        if (s >= n_sub) break;
+                        const int jj = j * SUB + s;
+                        const float ref = moved ? ((mode == kModeDynamic) ? m_used + fast_log2(lrun) : mrun) : ref0;
                         float gm = INFINITY;
                         if (want_margin) {
-                            float tm = row_valid ? t2 : -INFINITY;
+                            float tm = row_valid ? msub[s] - ref : -INFINITY;
 #pragma unroll
                             for (int o = 16; o > 0; o >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, o));
                             const uint32_t wm = sb + L::kWmax + 16 * q;
@@ -827,68 +844,26 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             named_bar_sync(1 + x, 128);
                         }
                         if (grp_leader && grp_valid) {
-                            if (a.skip_mask) a.skip_mask[tile_row + jj] = skip_s ? 1 : 0;
+                            if (a.skip_mask) a.skip_mask[tile_row + jj] = ((kept >> s) & 1u) ? 0 : 1;
                             if (want_margin) a.margin[tile_row + jj] = gm;
                         }
+                        if ((kept >> s) & 1u) { lrun += rsum[s]; mrun = fmaxf(mrun, msub[s]); moved = true; }
                     }
-                    if (skip_s) {
-                        ++n_skip;                            // a7: this decision tile leaves m, l, O untouched
-                        if (!kDebug || kept != 0u) {         // the MMA tile is retained: its parts go to the issuer, masked out
-                            tc_fence_before();               // (debug builds: parts ahead of the first retained sub-tile wait)
-#pragma unroll
-                            for (int c = s * CW; c < (s + 1) * CW; ++c) hand_over(c);
-                            handed = (s + 1) * CW;
-                        }
-                        continue;
-                    }
-                    if (kDebug && kept == 0u) {
-                        // debug builds take no vote on the whole tile: the first retained sub-tile tells the issuer and the
-                        // V warp that the MMA tile is kept
-                        tc_fence_before();
-                        if (lane == 0) {
-                            st_shared_u32(vote_w + 16 * q, vote_word(j, 2u));
-                            mbar_arrive(sb + L::kDec + 8 * q);
-                        }
-                        __syncwarp();
-                        if (spec) {                          // a speculative S_x(j+1) is in flight over these columns
-                            mbar_wait(sb + L::kSFull, sfpar);
-                            sfpar ^= 1u;
-                            tc_fence_after();
-                        }
-                        for (int c = handed; c < s * CW; ++c) hand_over(c);   // the skipped sub-tiles ahead of it (mask bits clear)
-                    }
-                    kept |= 1u << s;
-                    m_true = fmaxf(m_true, ms);
-                    if (!did_exp) {
-                        exp_sub(true);
-                    } else {
-                        tmem_wait_st();
-                        tc_fence_before();
-#pragma unroll
-                        for (int c = s * CW; c < (s + 1) * CW; ++c) hand_over(c);
-                    }
-                    handed = (s + 1) * CW;
-                    acc2 = add_f32x2(acc2, rs2);
-                    dirty = true;
                 }
-                if (kDebug && kept == 0u) {                  // (debug builds) every sub-tile skipped: the MMA tile is skipped
-                    tc_fence_before();
-                    if (lane == 0) {
-                        st_shared_u32(vote_w + 16 * q, vote_word(j, 1u));
-                        mbar_arrive(sb + L::kDec + 8 * q);
-                    }
-                    __syncwarp();
+                n_skip += __popc(valid & ~kept);             // a7 / a9: skipped decision tiles leave m, l, O untouched
+                if (!tile_kept) {
                     ++skip_run;
                     continue;
                 }
-                // (plain builds: a tile whose every sub-tile was skipped by the sequential rule after the vote round had
-                // kept it goes to the issuer with an empty mask: no P V step is issued)
                 skip_run = 0;
-                for (int c = handed; c < BC / 32; ++c) hand_over(c);   // (ragged tail: parts beyond the last decision tile)
-                fold();                                      // statistics for the next tile, behind the hand-over
+                // statistics for the next tile, behind the hand-over: the retained row sums in key order
+#pragma unroll
+                for (int s = 0; s < SUB; ++s) {
+                    if ((kept >> s) & 1u) { l += rsum[s]; m_true = fmaxf(m_true, msub[s]); }
+                }
+                if (mode == kModeDynamic) lse2 = m_used + fast_log2(l);
                 thr = ((mode == kModeDynamic) ? lse2 : m_true) + lam_row;
                 continue;
-                }   // !all_sure
             }
             // ---- predicate and all-rows vote (a4)
             bool skip_grp = false, keep_any = true, wskip = false;

@@ -95,11 +95,6 @@ __device__ __forceinline__ void named_bar_sync(uint32_t id, uint32_t nthreads) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// Producer side of a named barrier: counts the thread in and returns at once (the threads that need the outcome bar.sync).
-__device__ __forceinline__ void named_bar_arrive(uint32_t id, uint32_t nthreads) {
-    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
 // Barrier with an AND / OR reduction of one predicate per thread (all `nthreads` threads get the result).
 __device__ __forceinline__ bool named_bar_red_and(uint32_t id, uint32_t nthreads, bool pred) {
     uint32_t res;
