@@ -10,8 +10,9 @@
 //   warp  8     TMA producer for Q (once) and the K ring (runs ahead of the decisions)
 //   warp  9     tcgen05.mma issuer of slot 0 (one elected lane) and TMEM owner
 //   warp  10    TMA producer for the V ring: slot j % NV holds V_j.  DENSE: every tile.  Sparse modes: this warp
-//               reads both slots' votes on tile j and fetches V_j only if some slot keeps tile j (plus V_{j+1}
-//               speculatively after a kept tile); an unneeded tile completes its ring phase without a load
+//               reads both slots' votes on tile j and fetches V_j only if some slot keeps tile j (plus V_{j+1} ahead
+//               of its votes unless the last two tiles were skipped by both slots); an unneeded tile completes its
+//               ring phase without a load
 //   warp  11    tcgen05.mma issuer of slot 1
 // One issuer warp per slot: a thread that issues tcgen05.mma is held until its last MMA has been dispatched to the
 // tensor pipe, so with a single issuer every barrier wait and vote decode of one slot left the pipe idle; with two,
@@ -173,8 +174,9 @@ constexpr int kSpecRun = 2;
 // kDebug adds the optional skip_mask_out / margin_out parity outputs.
 // SUB == 0: the block-mass kernel of sparse_attn_block_mass (its own instantiation, so that the forward kernels carry none
 // of its code: a run-time branch for it inside the sparse kernels cost them 7-9 %).
-// SUB > 1 (sparse modes, G = 1): the decision tile is BR x (BC / SUB) keys -- SUB decisions per MMA tile, taken in
-// ascending key order with the statistics updated after every retained one (block size 32).
+// SUB > 1 (sparse modes, G = 1): the decision tile is BR x (BC / SUB) keys -- SUB decisions per MMA tile, equal to the
+// rule applied in ascending key order with the statistics updated after every retained one (block size
+// 32), taken in at most two vote rounds per MMA tile (see the SUB > 1 block of the softmax warpgroups).
 template <int D, int BC, int G, int NK, int NV, bool kSparse, bool kDebug, int SUB = 1>
 __global__ void __launch_bounds__(kNumThreads, 1)
 sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
@@ -386,8 +388,8 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             if (++kstage == NK) { kstage = 0; kphase ^= 1u; }
             uint32_t ppar[2] = {0u, 0u};                 // parity of p_half / p_ready: they advance on kept tiles only
             int skip_run[2] = {0, 0};                    // tiles in a row slot x has skipped, up to tile j-1
-            // Sparse modes, speculation: inside a run of skipped tiles the next S_x(j+1) = Q_x K_{j+1}^T is issued as
-            // soon as the softmax warps hold S_x(j) in registers (barrier s_read), without waiting for their vote:
+            // Sparse modes, speculation: inside a run of skipped tiles (kSpecRun or more in a row) the next S_x(j+1) =
+            // Q_x K_{j+1}^T is issued as soon as the softmax warps hold S_x(j) in registers (barrier s_read), without waiting for their vote:
             // the vote is then off the critical chain.  If tile j turns out to be kept, the softmax warps let the
             // speculative MMA finish before they write P_x over it, and S_x(j+1) is issued again after P_x V_j.
             // Scheduling only: no decision depends on it.
