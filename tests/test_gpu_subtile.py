@@ -107,3 +107,45 @@ def test_subtile_rejected_where_unsupported():
     with pytest.raises(sa.SparseAttnError) as e:           # DENSE mode takes no decisions
         sa.sparse_attn_fwd(q, q, q, out, None, 1, 1, 256, 128, sa.make_params(tile_q=128, tile_k=32), sa.MODE_DENSE, None)
     assert e.value.status == -4
+
+
+@pytest.mark.parametrize("tile_k", [32, 64])
+@pytest.mark.parametrize("mode", [MODE_DYNAMIC, MODE_FIXED])
+def test_subtile_decisions_that_depend_on_earlier_subtiles(parity, tile_k, mode):
+    """Inputs built so that, inside ONE 128-key MMA tile, the fate of a sub-tile depends on which earlier sub-tiles were
+    retained (Eq. 6 is sequential): every key of a sub-tile carries the same logit level, levels drawn so that most
+    sub-tiles pass the test against the statistics before the MMA tile and are then decided by the levels ahead of them
+    (the hypothesis bits of the kernel's second vote round).  Rows fall into four groups with shifted levels, one group per
+    warp, so the all-rows vote crosses warps.  Decisions, counts and outputs against the oracle."""
+    rng = np.random.default_rng([7, tile_k, mode])
+    D, N, S = 128, 1024 + 77, tile_k
+    n_sub = -(-N // S)
+    e0 = np.zeros(D, dtype=np.float32)
+    e0[0] = 1.0
+    worked = 0
+    for trial in range(6):
+        level = rng.uniform(0.0, 6.0, size=n_sub).astype(np.float32)          # logit level of every sub-tile
+        level[:: 128 // S] += rng.uniform(0.0, 3.0, size=len(level[:: 128 // S])).astype(np.float32)   # a strong first sub-tile
+        shift = np.repeat(rng.uniform(0.6, 1.0, size=4), 32)                      # four row groups (one per warp of a Q tile)
+        q = np.zeros((N, D), dtype=np.float32)
+        q[:, 0] = math.sqrt(D) * np.tile(shift, -(-N // 128))[:N]                 # logit(r, c) = shift_r * level_c (+ noise)
+        k = np.zeros((N, D), dtype=np.float32)
+        k[:, 0] = np.repeat(level, S)[:N]
+        k[:, 1:] = 0.02 * rng.standard_normal((N, D - 1)).astype(np.float32)
+        q[:, 1:] = 0.02 * rng.standard_normal((N, D - 1)).astype(np.float32)
+        v = rng.standard_normal((N, D)).astype(np.float32)
+        qb, kb, vb = (f32_to_bf16_bits(x)[None, None] for x in (q, k, v))
+        for lam in (-1.0, -2.5):
+            gpu = parity.run_gpu(qb, kb, vb, mode=mode, lam=lam, tile=128, tile_k=tile_k)
+            parity.check_stats(gpu, N, 128, tile_k)
+            rep = parity.compare_head(gpu, 0, qb[0, 0], kb[0, 0], vb[0, 0], tile=128, tile_k=tile_k, mode=mode, lam=lam)
+            assert rep.ok(), "\n".join(rep.failures[:10])
+            plain = parity.run_gpu(qb, kb, vb, mode=mode, lam=lam, tile=128, tile_k=tile_k, debug=False)
+            np.testing.assert_array_equal(plain.stats, gpu.stats)
+            np.testing.assert_array_equal(plain.out, gpu.out)
+            np.testing.assert_array_equal(plain.lse, gpu.lse)
+            # the case is only interesting if sub-tiles are skipped INSIDE retained MMA tiles
+            sk = gpu.skip[0].reshape(gpu.skip.shape[1], -1)
+            per_mma = sk[:, : (sk.shape[1] // (128 // S)) * (128 // S)].reshape(sk.shape[0], -1, 128 // S)
+            worked += int(((per_mma.sum(-1) > 0) & (per_mma.sum(-1) < 128 // S)).sum())
+    assert worked > 20, worked
