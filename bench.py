@@ -694,6 +694,14 @@ def main():
 
     sampler.__exit__()
     clocks = sampler.summary()
+    if selectors is not None and clocks.get("sm_mhz"):
+        # the block-sum pre-pass has one ex2 per logit and no P V to hide it behind: its roofline is the MUFU pipe
+        # (16 ex2 / clk / SM, 148 SMs), i.e. 2 D FLOP of Q K^T per ex2; clock = the median sampled in the
+        # timed loops of this run
+        peak = 16.0 * 148 * clocks["sm_mhz"] * 1e6 * 2.0 * cfg.D / 1e12
+        selectors["block_mass_roofline"] = {"bound": "alu", "pipe": "MUFU ex2, 16 / clk / SM", "achieved": selectors["block_mass_tflops"],
+                                            "peak": peak, "unit": "TFLOP/s of Q K^T", "frac": selectors["block_mass_tflops"] / peak,
+                                            "sm_mhz": clocks["sm_mhz"]}
 
     # ------------------------------------------------------------------ end-to-end through the host-buffer C entry point
     qb, kb, vb = host_data[args.config]
