@@ -466,12 +466,9 @@ int sparse_attn_reorder_tokens(const void* src, void* dst, int B, int H, int N, 
     if (s0 < d0 + bytes && d0 < s0 + bytes) return fail(SPARSE_ATTN_ERR_PARAMS, "src and dst overlap");
     int rc = check_device();
     if (rc) return rc;
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        CUDA_TRY(cudaGetDevice(&dev));
-        CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    }
+    int n_sm = 0, dev = 0;                                   // per call: the current device may differ between calls
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     const long long rows = static_cast<long long>(B) * H * N;
     const int lanes = D / 8;                                 // 16 bytes per thread
     const long long blocks_needed = (rows + (256 / lanes) * 4 - 1) / ((256 / lanes) * 4);
@@ -494,7 +491,7 @@ int sparse_attn_recall_stats(const float* lse_retained, const float* lse_dense, 
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     dsa::stats_init_kernel<<<1, 1, 0, st>>>(stats_out, INFINITY, 0.0);
-    const int grid = static_cast<int>(std::min<int64_t>((n_rows + 255) / 256, 148 * 8));
+    const int grid = static_cast<int>(std::min<int64_t>((n_rows + 255) / 256, 148 * 8));   // (8 CTAs per B200 SM)
     dsa::recall_stats_kernel<<<grid, 256, 0, st>>>(lse_retained, lse_dense, n_rows, stats_out);
     CUDA_TRY(cudaGetLastError());
     g_reorder_launches.fetch_add(2);
