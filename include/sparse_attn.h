@@ -67,13 +67,7 @@ typedef struct sparse_attn_params {
                                key order, the statistics are updated after every retained one, and exp, row sum and
                                P V are skipped per decision tile.  T_c below is then ceil(N / tile_k).  With these
                                narrow tiles lambda must be <= 0 (the softmax stabiliser follows the max of the whole
-                               128-key MMA tile, which only a non-positive threshold is certain to retain).  For the same
-                               reason the statistics of a row inside one 128-key MMA tile are held relative to that
-                               tile's row maximum in fp32: if a row's logits rise by more than ~126 log2 units (87 in
-                               natural-log units) above its running log-sum-exp INSIDE one MMA tile, the references of
-                               that row's other narrow tiles in it underflow and the row votes "keep" on them -- a
-                               decision tile the rule would skip may then be retained (never the reverse: recall is
-                               not reduced).  Logits bounded by |s| <= 87 / 2 cannot trigger it. */
+                               128-key MMA tile, which only a non-positive threshold is certain to retain). */
     void* stream;           /* cudaStream_t to launch on; NULL = the default stream */
     uint8_t* skip_mask_out; /* optional, device, [B, H, T_r, T_c] bytes, 1 = tile skipped, fully overwritten.
                                T_r = ceil(N / tile_q), T_c = ceil(N / tile_k).  NULL in timed runs. */

@@ -695,6 +695,37 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 float rsum[SUB];                             // row sums of the exponentiated sub-tiles
 #pragma unroll
                 for (int s = 0; s < SUB; ++s) rsum[s] = 0.f;
+                // The reference of a row once the sub-tiles of set h (all before s) are retained: LSE(h) = m + log2(l +
+                // sum_{i in h} rsum_i), summed in key order exactly as the statistics are updated below (Eq. 6); FIXED:
+                // max(m, max_{i in h} msub_i).  `wide` rows -- the tile's row max sits more than 100 log2 units above the
+                // row's reference before the tile, so that sums relative to that max would leave the fp32 range -- combine
+                // log-sums instead: lsub_i = msub_i + log2(sum_c 2^(s_c - msub_i)), each relative to its own sub-tile.
+                bool wide = false;
+                float lsub[SUB];
+#pragma unroll
+                for (int s = 0; s < SUB; ++s) lsub[s] = -INFINITY;
+                auto ref_after = [&](int s, uint32_t h) {
+                    if (mode == kModeDynamic) {
+                        if (wide) {
+                            float M = ref0;
+#pragma unroll
+                            for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) M = fmaxf(M, lsub[i]);
+                            if (M == -INFINITY) return M;
+                            float acc = fast_exp2(ref0 - M);
+#pragma unroll
+                            for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) acc += fast_exp2(lsub[i] - M);
+                            return M + fast_log2(acc);
+                        }
+                        float lh = l;
+#pragma unroll
+                        for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) lh += rsum[i];
+                        return m_used + fast_log2(lh);
+                    }
+                    float ref = m_true;
+#pragma unroll
+                    for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) ref = fmaxf(ref, msub[i]);
+                    return ref;
+                };
                 if (tile_kept) {
                     if (spec) {                              // kept after all: let the speculative S_x(j+1) land first
                         mbar_wait(sb + L::kSFull, sfpar);
@@ -737,21 +768,6 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         if (c == BC / 32 - 1) mbar_arrive(sb + L::kPReady);
                         else mbar_arrive(sb + L::kPPart + 8 * c);
                     };
-                    // the reference of a row once the sub-tiles of set h (all before s) are retained: LSE(h) = m + log2(l +
-                    // sum_{i in h} rsum_i), summed in key order exactly as the statistics are updated below (Eq. 6);
-                    // FIXED: max(m, max_{i in h} msub_i)
-                    auto ref_after = [&](int s, uint32_t h) {
-                        if (mode == kModeDynamic) {
-                            float lh = l;
-#pragma unroll
-                            for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) lh += rsum[i];
-                            return m_used + fast_log2(lh);
-                        }
-                        float ref = m_true;
-#pragma unroll
-                        for (int i = 0; i < SUB - 1; ++i) if (i < s && ((h >> i) & 1u)) ref = fmaxf(ref, msub[i]);
-                        return ref;
-                    };
                     // a5 for every candidate: all of them are exponentiated in one straight pass -- an open sub-tile that
                     // round 2 skips has cost its ex2 work and nothing else (its P columns are never read)
 #pragma unroll
@@ -776,6 +792,21 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                         } else {                             // skipped in round 1 (or beyond the last key): masked out
 #pragma unroll
                             for (int c = s * CW; c < (s + 1) * CW; ++c) hand_over(c);
+                        }
+                    }
+                    if (mode == kModeDynamic && (open != 0u || kDebug)) {
+                        wide = m_used - ref0 > 100.f;        // (also every row of the first tile: ref0 = -inf)
+                        if (__any_sync(0xffffffffu, wide)) {
+#pragma unroll
+                            for (int i = 0; i < SUB - 1; ++i) {
+                                if ((cand >> i) & 1u) {
+                                    const float nm = -msub[i];
+                                    float acc = 0.f;
+#pragma unroll
+                                    for (int c = i * W; c < (i + 1) * W; ++c) acc += fast_exp2(fmaf(S_AT(c), scale_log2, nm));
+                                    lsub[i] = msub[i] + fast_log2(acc);
+                                }
+                            }
                         }
                     }
                     if (open != 0u) {
@@ -824,13 +855,12 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                 if (kDebug) {
                     // parity outputs: the decision of every sub-tile and its margin g = max_r t_r - lambda, t evaluated against
                     // the reference the sequential rule saw (the retained sub-tiles before it)
-                    float lrun = l, mrun = m_true;
                     bool moved = false;
 #pragma unroll
                     for (int s = 0; s < SUB; ++s) {
                         if (s >= n_sub) break;
                         const int jj = j * SUB + s;
-                        const float ref = moved ? ((mode == kModeDynamic) ? m_used + fast_log2(lrun) : mrun) : ref0;
+                        const float ref = moved ? ref_after(s, kept & ((1u << s) - 1u)) : ref0;
                         float gm = INFINITY;
                         if (want_margin) {
                             float tm = row_valid ? msub[s] - ref : -INFINITY;
@@ -849,7 +879,7 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
                             if (a.skip_mask) a.skip_mask[tile_row + jj] = ((kept >> s) & 1u) ? 0 : 1;
                             if (want_margin) a.margin[tile_row + jj] = gm;
                         }
-                        if ((kept >> s) & 1u) { lrun += rsum[s]; mrun = fmaxf(mrun, msub[s]); moved = true; }
+                        if ((kept >> s) & 1u) moved = true;
                     }
                 }
                 n_skip += __popc(valid & ~kept);             // a7 / a9: skipped decision tiles leave m, l, O untouched
