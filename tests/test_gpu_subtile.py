@@ -149,3 +149,28 @@ def test_subtile_decisions_that_depend_on_earlier_subtiles(parity, tile_k, mode)
             per_mma = sk[:, : (sk.shape[1] // (128 // S)) * (128 // S)].reshape(sk.shape[0], -1, 128 // S)
             worked += int(((per_mma.sum(-1) > 0) & (per_mma.sum(-1) < 128 // S)).sum())
     assert worked > 20, worked
+
+
+def test_subtile_logits_that_leave_the_fp32_range_inside_one_mma_tile(parity):
+    """Random-walk Q / K with logits of several hundred nats: rows whose logits rise by more than 126 log2 units above their
+    running LSE inside ONE 128-key MMA tile.  Sums relative to the tile's row max underflow there; the kernel's references
+    for such rows come from per-sub-tile log-sums instead.  Decisions and margins against the oracle (a soak run found the
+    case as margins off by 0.4 - 3.8 nats before that branch existed)."""
+    N, D, H, gain, lam = 1423, 128, 3, 2.9630839477090753, -5.9537085225695545
+    rng = np.random.default_rng(793270137)
+    q = rng.standard_normal((1, H, N, D), dtype=np.float32) * gain
+    k = rng.standard_normal((1, H, N, D), dtype=np.float32)
+    base = np.cumsum(rng.standard_normal((1, H, N, D), dtype=np.float32), axis=2) / 8.0
+    q = (base + 0.3 * q) * gain
+    k = base + 0.3 * k
+    v = rng.standard_normal((1, H, N, D), dtype=np.float32)
+    qb, kb, vb = (f32_to_bf16_bits(x) for x in (q, k, v))
+    for tile_k in (32, 64):
+        gpu = parity.run_gpu(qb, kb, vb, mode=MODE_DYNAMIC, lam=lam, tile=128, tile_k=tile_k)
+        parity.check_stats(gpu, N, 128, tile_k)
+        rep = parity.ParityReport()
+        for h in range(H):
+            parity.compare_head(gpu, h, qb[0, h], kb[0, h], vb[0, h], tile=128, tile_k=tile_k, mode=MODE_DYNAMIC, lam=lam,
+                                report=rep)
+        assert rep.ok(), "\n".join(rep.failures[:10])
+        assert rep.max_margin_abs < 1e-3
