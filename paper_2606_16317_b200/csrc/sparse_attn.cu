@@ -242,7 +242,7 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     const size_t head_elems = static_cast<size_t>(N) * D;
     const size_t T_r = (N + r.tile_q - 1) / r.tile_q, T_c = (N + r.tile_k - 1) / r.tile_k;
     const size_t head_tiles = T_r * T_c;
-    constexpr int kMaxChunks = 8;
+    constexpr int kMaxChunks = 20;      // (config 3: 2 heads = 4 whole waves per chunk; 8 chunks left 3 ms of copy head and tail exposed)
     const int n_chunks = static_cast<int>(std::min<size_t>(BH, kMaxChunks));
     cudaStream_t st = r.stream;
     cudaStream_t s_in = nullptr, s_out = nullptr, s_k[2] = {nullptr, nullptr};
