@@ -7,8 +7,10 @@
  * (Q_i, K_j) tile is skipped (section 3.1, Eq. 5-6).  No mask pre-pass.
  *
  * All entry points are plain C, never throw, never exit the process, and allocate no persistent
- * device memory.  There is no CPU fallback: on a machine without an sm_100 device every compute
- * call fails with SPARSE_ATTN_ERR_DEVICE.
+ * device memory (the one fixed exception is the 16 MiB static array behind
+ * sparse_attn_row_topk_curve_static, which is part of the library's device image).  There is no
+ * CPU fallback: on a machine without an sm_100 device every compute call fails with
+ * SPARSE_ATTN_ERR_DEVICE.
  */
 #ifndef SPARSE_ATTN_H_
 #define SPARSE_ATTN_H_
@@ -246,6 +248,43 @@ int sparse_attn_output_error(const void* out_a, const void* out_b, int64_t n_ele
 int sparse_attn_row_topk_curve(const void* q, const void* k, const void* v, int B, int H, int N, int D, float softmax_scale,
                                const int32_t* rows, int n_rows, const int32_t* keep_counts, int n_keep,
                                double* kurtosis_out, double* recall_out, double* mae_out, void* stream);
+
+/*
+ * sparse_attn_row_topk_curve for callers that must not allocate device memory.
+ *
+ * Who needs it: a host program that has already given the whole GPU to another allocator (an inference server that
+ * reserves all free HBM for its cache at start-up, so that a later cudaMalloc / cudaMallocAsync simply fails with
+ * out-of-memory), or one whose request path is forbidden to touch the driver's allocator because cudaMalloc and
+ * cudaFree may stall every stream of the device.  sparse_attn_row_topk_curve above takes n_rows * N * 4 bytes plus two
+ * small index buffers from the stream-ordered pool on every call; this entry point takes nothing: it calls no
+ * cudaMalloc*, no cudaFree* and no library routine that allocates.
+ *
+ * Same computation, same kernel, same arguments and same results as sparse_attn_row_topk_curve (q, k, v and the three
+ * outputs are the caller's device buffers, rows / keep_counts the caller's host arrays).  The only difference is where the
+ * kernel's working memory lives: one fixed array inside the library's device image,
+ *     SPARSE_ATTN_STATIC_SCRATCH_FLOATS fp32 (16 MiB: one line of N exponentials per sampled row)
+ *     + SPARSE_ATTN_STATIC_MAX_ROWS (bh, r) pairs + SPARSE_ATTN_STATIC_MAX_KEEP keep counts  (32 KiB),
+ * which every GPU that loads this library holds from the moment its code is loaded until the process exits.
+ * Limits, checked before anything is enqueued (SPARSE_ATTN_ERR_SHAPE, nothing written):
+ *     (int64) n_rows * N <= SPARSE_ATTN_STATIC_SCRATCH_FLOATS,  n_rows <= SPARSE_ATTN_STATIC_MAX_ROWS,
+ *     n_keep <= SPARSE_ATTN_STATIC_MAX_KEEP     (e.g. 128 rows at N = 32760, 55 rows at N = 75600; split larger samples
+ *     into several calls, one after the other).
+ * Set-up: the first call on each device (made with that device current) looks up the array's device address once and
+ * remembers it; make that first call before any stream capture begins.  Later calls on the device do no set-up.
+ * Sharing: there is ONE array per device and every call uses it.  Two calls whose kernels may overlap on the GPU (two
+ * streams, or two host threads) corrupt each other's results -- run them in stream order or serialise them yourself.
+ * The array keeps the previous call's contents; that is harmless here, because each call overwrites the row list, the K
+ * list and every element of its rows' lines before anything reads them, so nothing has to be cleared between calls.
+ * Like sparse_attn_row_topk_curve it copies rows / keep_counts to the device, synchronises `stream` once (so the caller
+ * may reuse them), enqueues one kernel and returns; the caller synchronises before reading the outputs.
+ * Errors: those of sparse_attn_row_topk_curve, plus SPARSE_ATTN_ERR_SHAPE beyond the limits above.
+ */
+#define SPARSE_ATTN_STATIC_SCRATCH_FLOATS (4u << 20)
+#define SPARSE_ATTN_STATIC_MAX_ROWS 2048
+#define SPARSE_ATTN_STATIC_MAX_KEEP 4096
+int sparse_attn_row_topk_curve_static(const void* q, const void* k, const void* v, int B, int H, int N, int D,
+                                      float softmax_scale, const int32_t* rows, int n_rows, const int32_t* keep_counts,
+                                      int n_keep, double* kurtosis_out, double* recall_out, double* mae_out, void* stream);
 
 /* Static string for a status code. */
 const char* sparse_attn_status_string(int status);

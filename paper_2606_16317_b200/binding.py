@@ -30,6 +30,7 @@ EXPORTED_SYMBOLS = (
     "sparse_attn_recall_stats",
     "sparse_attn_output_error",
     "sparse_attn_row_topk_curve",
+    "sparse_attn_row_topk_curve_static",
     "sparse_attn_brick_permutation",
     "sparse_attn_reorder_tokens",
     "sparse_attn_select_blocks",
@@ -97,6 +98,8 @@ def _load():
         lib.sparse_attn_row_topk_curve.restype = ctypes.c_int
         lib.sparse_attn_row_topk_curve.argtypes = [ctypes.c_void_p] * 3 + [ctypes.c_int] * 4 + [ctypes.c_float, ctypes.c_void_p,
                                                    ctypes.c_int, ctypes.c_void_p, ctypes.c_int] + [ctypes.c_void_p] * 4
+        lib.sparse_attn_row_topk_curve_static.restype = ctypes.c_int
+        lib.sparse_attn_row_topk_curve_static.argtypes = lib.sparse_attn_row_topk_curve.argtypes
         lib.sparse_attn_select_blocks.restype = ctypes.c_int
         lib.sparse_attn_select_blocks.argtypes = [ctypes.c_void_p, ctypes.c_void_p] + [ctypes.c_int] * 5 + [
             ctypes.c_double, ctypes.c_void_p]
@@ -267,6 +270,28 @@ def sparse_attn_row_topk_curve(q, k, v, B, H, N, D, rows, keep_counts, kurtosis_
     rc = _load().sparse_attn_row_topk_curve(_ptr(q), _ptr(k), _ptr(v), int(B), int(H), int(N), int(D), float(softmax_scale),
                                             _ptr(rows), n_rows, _ptr(keep_counts), n_keep, _ptr(kurtosis_out),
                                             _ptr(recall_out), _ptr(mae_out), _ptr(stream))
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
+
+
+# limits of the allocation-free entry point (include/sparse_attn.h: SPARSE_ATTN_STATIC_*)
+STATIC_SCRATCH_FLOATS, STATIC_MAX_ROWS, STATIC_MAX_KEEP = 4 << 20, 2048, 4096
+
+
+def sparse_attn_row_topk_curve_static(q, k, v, B, H, N, D, rows, keep_counts, kurtosis_out, recall_out, mae_out,
+                                      softmax_scale=0.0, stream=None):
+    """C entry point `sparse_attn_row_topk_curve_static`: the Appendix A.1 row curve for hosts that cannot allocate device
+    memory -- a process whose HBM has all been handed to another allocator (any cudaMalloc would fail), or a request path
+    that must not call the driver's allocator.  Same arguments and results as `sparse_attn_row_topk_curve`; the kernel's
+    working memory is a fixed 16 MiB array inside the library, so n_rows * N <= STATIC_SCRATCH_FLOATS, n_rows <=
+    STATIC_MAX_ROWS, n_keep <= STATIC_MAX_KEEP (SparseAttnError with status -2 beyond).  Every call on a device shares that
+    one array: calls that may overlap on the GPU race.  The first call on a device looks the array's address up; make it
+    before any stream capture."""
+    n_rows, n_keep = int(rows.shape[0]), int(keep_counts.shape[0])
+    rc = _load().sparse_attn_row_topk_curve_static(_ptr(q), _ptr(k), _ptr(v), int(B), int(H), int(N), int(D),
+                                                   float(softmax_scale), _ptr(rows), n_rows, _ptr(keep_counts), n_keep,
+                                                   _ptr(kurtosis_out), _ptr(recall_out), _ptr(mae_out), _ptr(stream))
     if rc != 0:
         raise SparseAttnError(rc, last_error())
     return rc

@@ -564,6 +564,94 @@ int sparse_attn_row_topk_curve(const void* q, const void* k, const void* v, int 
     return 0;
 }
 
+// ---- sparse_attn_row_topk_curve without any allocation ---------------------------------------------------------------
+// Working memory of row_topk_curve_kernel for callers that cannot allocate on the device (a host that has handed all
+// of HBM to another allocator, or whose request path must stay away from cudaMalloc / cudaFree): a fixed array in this
+// translation unit's device image.  Layout: [0, 16 MiB) fp32 lines of exponentials, then the (bh, r) pairs, then the K list.
+// g_curve_static is a HOST-side stand-in in host code -- never pass it to a kernel or a memcpy; the device address comes
+// from cudaGetSymbolAddress (curve_static_base below), once per device.
+constexpr size_t kCurveStaticLineBytes = sizeof(float) * static_cast<size_t>(SPARSE_ATTN_STATIC_SCRATCH_FLOATS);
+constexpr size_t kCurveStaticRowBytes = sizeof(int32_t) * 2 * SPARSE_ATTN_STATIC_MAX_ROWS;
+constexpr size_t kCurveStaticKeepBytes = sizeof(int32_t) * SPARSE_ATTN_STATIC_MAX_KEEP;
+static __device__ __align__(256) unsigned char g_curve_static[kCurveStaticLineBytes + kCurveStaticRowBytes + kCurveStaticKeepBytes];
+
+namespace {
+constexpr int kCurveStaticMaxDevices = 64;
+std::atomic<unsigned char*> g_curve_static_base[kCurveStaticMaxDevices];
+
+// Device address of g_curve_static on the CURRENT device: looked up on the first call per device, remembered afterwards
+// (two threads racing through the first call both store the same address).
+int curve_static_base(unsigned char** base) {
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    const bool cacheable = dev >= 0 && dev < kCurveStaticMaxDevices;
+    if (cacheable) {
+        unsigned char* known = g_curve_static_base[dev].load(std::memory_order_acquire);
+        if (known) { *base = known; return 0; }
+    }
+    void* ptr = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress(&ptr, g_curve_static));
+    if (!ptr) return fail(SPARSE_ATTN_ERR_CUDA, "cudaGetSymbolAddress returned a NULL address for the static scratch array");
+    if (cacheable) g_curve_static_base[dev].store(static_cast<unsigned char*>(ptr), std::memory_order_release);
+    *base = static_cast<unsigned char*>(ptr);
+    return 0;
+}
+}  // namespace
+
+int sparse_attn_row_topk_curve_static(const void* q, const void* k, const void* v, int B, int H, int N, int D,
+                                      float softmax_scale, const int32_t* rows, int n_rows, const int32_t* keep_counts,
+                                      int n_keep, double* kurtosis_out, double* recall_out, double* mae_out, void* stream) {
+    g_last_error[0] = '\0';
+    if (!q || !k || !v || !rows || !keep_counts || !kurtosis_out || !recall_out || !mae_out)
+        return fail(SPARSE_ATTN_ERR_NULL_POINTER, "q, k, v, rows, keep_counts and the three outputs must not be NULL");
+    if (B <= 0 || H <= 0 || N <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "B, H, N must be positive (got %d, %d, %d)", B, H, N);
+    if (N > (1 << 24)) return fail(SPARSE_ATTN_ERR_SHAPE, "N = %d exceeds 2^24", N);
+    if (D != 64 && D != 128) return fail(SPARSE_ATTN_ERR_HEAD_DIM, "D = %d not in {64, 128}", D);
+    if (n_rows <= 0 || n_keep <= 0) return fail(SPARSE_ATTN_ERR_SHAPE, "n_rows and n_keep must be positive (got %d, %d)", n_rows, n_keep);
+    if (n_rows > SPARSE_ATTN_STATIC_MAX_ROWS || n_keep > SPARSE_ATTN_STATIC_MAX_KEEP)
+        return fail(SPARSE_ATTN_ERR_SHAPE, "n_rows = %d / n_keep = %d exceed the static limits of %d rows and %d K values per call",
+                    n_rows, n_keep, SPARSE_ATTN_STATIC_MAX_ROWS, SPARSE_ATTN_STATIC_MAX_KEEP);
+    if (static_cast<long long>(n_rows) * N > static_cast<long long>(SPARSE_ATTN_STATIC_SCRATCH_FLOATS))
+        return fail(SPARSE_ATTN_ERR_SHAPE, "n_rows * N = %lld exceeds the static scratch of %u floats (16 MiB): at N = %d pass at most "
+                    "%d rows per call, or use sparse_attn_row_topk_curve, which allocates",
+                    static_cast<long long>(n_rows) * N, SPARSE_ATTN_STATIC_SCRATCH_FLOATS, N,
+                    static_cast<int>(SPARSE_ATTN_STATIC_SCRATCH_FLOATS / static_cast<unsigned>(N)));
+    if (!(softmax_scale >= 0.f) || std::isinf(softmax_scale))
+        return fail(SPARSE_ATTN_ERR_PARAMS, "softmax_scale must be finite and >= 0 (0 = 1/sqrt(D))");
+    for (int i = 0; i < n_rows; ++i)
+        if (rows[2 * i] < 0 || rows[2 * i] >= B * H || rows[2 * i + 1] < 0 || rows[2 * i + 1] >= N)
+            return fail(SPARSE_ATTN_ERR_PARAMS, "rows[%d] = (%d, %d) outside [0, B*H) x [0, N)", i, rows[2 * i], rows[2 * i + 1]);
+    for (int i = 0; i < n_keep; ++i)
+        if (keep_counts[i] < 1 || keep_counts[i] > N)
+            return fail(SPARSE_ATTN_ERR_PARAMS, "keep_counts[%d] = %d outside [1, N]", i, keep_counts[i]);
+    if ((reinterpret_cast<uintptr_t>(q) | reinterpret_cast<uintptr_t>(k) | reinterpret_cast<uintptr_t>(v)) & 15u)
+        return fail(SPARSE_ATTN_ERR_ALIGNMENT, "q, k and v must be 16-byte aligned");
+    int rc = check_device();
+    if (rc) return rc;
+    unsigned char* base = nullptr;                           // (first call on this device: the one-time address look-up)
+    if ((rc = curve_static_base(&base))) return rc;
+    float* lines = reinterpret_cast<float*>(base);
+    int32_t* d_rows = reinterpret_cast<int32_t*>(base + kCurveStaticLineBytes);
+    int32_t* d_keep = reinterpret_cast<int32_t*>(base + kCurveStaticLineBytes + kCurveStaticRowBytes);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // Nothing in the array has to start at zero: the two lists are overwritten here, and the kernel stores all N logits of
+    // a row's line before it reads any of them.  What the previous call left behind is never looked at.
+    CUDA_TRY(cudaMemcpyAsync(d_rows, rows, sizeof(int32_t) * 2 * n_rows, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(d_keep, keep_counts, sizeof(int32_t) * n_keep, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));                     // rows / keep_counts may be pageable: the caller may reuse them now
+    const float scale = softmax_scale > 0.f ? softmax_scale : 1.0f / std::sqrt(static_cast<float>(D));
+    auto qp = static_cast<const __nv_bfloat16*>(q), kp = static_cast<const __nv_bfloat16*>(k), vp = static_cast<const __nv_bfloat16*>(v);
+    if (D == 128)
+        dsa::row_topk_curve_kernel<128><<<n_rows, dsa::kRowCurveThreads, 0, st>>>(qp, kp, vp, N, scale, d_rows, d_keep, n_keep, lines,
+                                                                                  kurtosis_out, recall_out, mae_out);
+    else
+        dsa::row_topk_curve_kernel<64><<<n_rows, dsa::kRowCurveThreads, 0, st>>>(qp, kp, vp, N, scale, d_rows, d_keep, n_keep, lines,
+                                                                                 kurtosis_out, recall_out, mae_out);
+    CUDA_TRY(cudaGetLastError());
+    g_reorder_launches.fetch_add(1);
+    return 0;
+}
+
 double sparse_attn_lambda_from_recall(double recall, int N) { return std::log((1.0 - recall) / N); }
 
 double sparse_attn_lambda_from_preal(double p_real, int tile_k, int N) {
