@@ -57,6 +57,16 @@ def run_gpu(q_bits: np.ndarray, k_bits: np.ndarray, v_bits: np.ndarray, *, mode:
                      margin.cpu().numpy().reshape(B * H, T, Tc) if debug else None)
 
 
+def scale_free_out_tol(v64: np.ndarray):
+    """Output allowance that holds for ANY input scale: the kernel rounds P to bf16 before P V
+    (relative 2^-8 per probability, so at most 2^-8 max_c |v_cd| in column d after the division by the unrounded row
+    sum) and rounds the output to bf16 (2^-8 |o|); 1e-3 covers the fp32 accumulation, ex2.approx and the FMA-pipe
+    polynomial.  On the contract workloads (|o| << 1, |v| <= 4.5) this is the 2e-2 of BASELINE.json."""
+    vmax = np.abs(v64).max(axis=0)                             # [D]
+    mean_tol = OUT_MEAN_ABS * max(1.0, float(vmax.max()) / 4.0)
+    return (lambda o_ref: 2.0 ** -8 * (np.abs(o_ref) + vmax[None, :]) + 1e-3), mean_tol
+
+
 @dataclass
 class ParityReport:
     tiles_checked: int = 0
@@ -81,8 +91,16 @@ class ParityReport:
 
 def compare_head(gpu: GpuResult, bh: int, q_bits, k_bits, v_bits, *, tile: int, mode: int, lam: float,
                  qtiles: Optional[Sequence[int]] = None, report: Optional[ParityReport] = None,
-                 scale: Optional[float] = None, tile_k: Optional[int] = None) -> ParityReport:
-    """Compare one head of a GPU run with the oracle on the given decision tiles (all if None)."""
+                 scale: Optional[float] = None, tile_k: Optional[int] = None, out_tol=None,
+                 margin_tol: float = MARGIN_TOL) -> ParityReport:
+    """Compare one head of a GPU run with the oracle on the given decision tiles (all if None).
+
+    out_tol: None = BASELINE.json's output bounds (OUT_MAX_ABS / OUT_MEAN_ABS, which hold on the contract workloads);
+    otherwise `scale_free_out_tol(v)`: (per-column max-abs allowance function of o_ref, mean-abs allowance) for inputs
+    whose values leave the contract's range.
+    margin_tol: the decision / margin tolerance; BASELINE.json's 1e-3 logit units by default, which presumes logits of the
+    contract's size -- S is an fp32 number, so a margin between logits of +-1500 nats carries a few ulp(1500) = 1e-4
+    each; tests that draw such inputs pass 1e-3 + 1e-6 max|S|."""
     rep = report if report is not None else ParityReport()
     N, D = q_bits.shape
     T = -(-N // tile)
@@ -107,13 +125,13 @@ def compare_head(gpu: GpuResult, bh: int, q_bits, k_bits, v_bits, *, tile: int, 
             rep.disagreements += len(dis)
             first = int(dis[0])
             g_first = free.margin[t, first]                    # same state on both sides up to `first`
-            if abs(g_first) <= MARGIN_TOL:
+            if abs(g_first) <= margin_tol:
                 rep.near_margin_disagreements += 1
             else:
                 rep.failures.append(f"head {bh} qtile {i}: first disagreement at j={first} has margin {g_first:.3e}")
             # replay: the GPU's decision must equal (g < 0) wherever |g| > tol, g evaluated from the GPU's kept set
             g = replay.margin[d]
-            must = np.abs(g) > MARGIN_TOL
+            must = np.abs(g) > margin_tol
             bad = must & ((g < 0) != (gskip[t] != 0))
             if bad.any():
                 j = int(np.nonzero(bad)[0][0])
@@ -131,10 +149,20 @@ def compare_head(gpu: GpuResult, bh: int, q_bits, k_bits, v_bits, *, tile: int, 
         rep.mean_abs_sum += float(err.sum())
         rep.mean_abs_n += err.size
         rep.max_lse_abs = max(rep.max_lse_abs, float(np.abs(l_gpu - l_ref).max()))
-        if err.max() > OUT_MAX_ABS:
-            rep.failures.append(f"head {bh} qtile {i}: out max-abs {err.max():.3e} > {OUT_MAX_ABS}")
-        if err.mean() > OUT_MEAN_ABS:
-            rep.failures.append(f"head {bh} qtile {i}: out mean-abs {err.mean():.3e} > {OUT_MEAN_ABS}")
+        if out_tol is None:
+            if err.max() > OUT_MAX_ABS:
+                rep.failures.append(f"head {bh} qtile {i}: out max-abs {err.max():.3e} > {OUT_MAX_ABS}")
+            if err.mean() > OUT_MEAN_ABS:
+                rep.failures.append(f"head {bh} qtile {i}: out mean-abs {err.mean():.3e} > {OUT_MEAN_ABS}")
+        else:
+            elem_tol, mean_tol = out_tol
+            over = err - elem_tol(o_ref)
+            if over.max() > 0:
+                r, c = np.unravel_index(int(over.argmax()), over.shape)
+                rep.failures.append(f"head {bh} qtile {i}: out err {err[r, c]:.3e} at |o| = {abs(o_ref[r, c]):.3f} exceeds the "
+                                    f"scale-free bound {elem_tol(o_ref)[r, c]:.3e}")
+            if err.mean() > mean_tol:
+                rep.failures.append(f"head {bh} qtile {i}: out mean-abs {err.mean():.3e} > {mean_tol:.3e}")
         if np.abs(l_gpu - l_ref).max() > LSE_ABS:
             rep.failures.append(f"head {bh} qtile {i}: lse abs err {np.abs(l_gpu - l_ref).max():.3e} > {LSE_ABS}")
         # margins the GPU evaluated (debug output) against the oracle's, same kept set
@@ -145,8 +173,8 @@ def compare_head(gpu: GpuResult, bh: int, q_bits, k_bits, v_bits, *, tile: int, 
         elif fin.any():
             merr = float(np.abs(gm[fin] - g_ref[fin]).max())
             rep.max_margin_abs = max(rep.max_margin_abs, merr)
-            if merr > MARGIN_TOL:
-                rep.failures.append(f"head {bh} qtile {i}: margin abs err {merr:.3e} > {MARGIN_TOL}")
+            if merr > margin_tol:
+                rep.failures.append(f"head {bh} qtile {i}: margin abs err {merr:.3e} > {margin_tol}")
     return rep
 
 
