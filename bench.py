@@ -726,6 +726,20 @@ def main():
     barrier()
     h2d = 3 * hq.numel() * 2
     d2h = hout.numel() * 2 + hlse.numel() * 4 + hstats.numel() * 8
+    # the timed host-buffer call must have produced what the device entry produces on the same inputs, bit for bit
+    # (20 head chunks over four streams against one launch); checked outside the timed region
+    sa.sparse_attn_release_scratch()
+    dq, dk, dv = (x.cuda().view(torch.bfloat16) for x in (hq, hk, hv))
+    dout = torch.empty_like(dq)
+    dlse = torch.empty((cfg.B, cfg.H, cfg.N), dtype=torch.float32, device="cuda")
+    dstats = torch.zeros((cfg.B, cfg.H, 2), dtype=torch.int64, device="cuda")
+    sa.sparse_attn_fwd(dq, dk, dv, dout, dlse, cfg.B, cfg.H, cfg.N, cfg.D, p, sa.MODE_DYNAMIC, dstats)
+    torch.cuda.synchronize()
+    e2e_equal = (torch.equal(dout.view(torch.int16).cpu(), hout) and torch.equal(dlse.cpu(), hlse)
+                 and torch.equal(dstats.cpu(), hstats))
+    if not e2e_equal:
+        raise RuntimeError("sparse_attn_fwd_host and sparse_attn_fwd disagree on the bench workload")
+    del dq, dk, dv, dout, dlse, dstats
 
     if rank != 0:
         if dist is not None:
@@ -780,7 +794,8 @@ def main():
         "cpu_baseline": cpu_baseline,
         "e2e": {"value": dense_flop(BH * world, cfg.N, cfg.D) / e2e_s / 1e12, "unit": UNIT,
                 "ms_per_step": e2e_s * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "path": "sparse_attn_fwd_host: pinned host buffers, H2D + kernel + D2H pipelined over head chunks"},
+                "path": "sparse_attn_fwd_host: pinned host buffers, H2D + kernel + D2H pipelined over head chunks",
+                "equals_device_entry": bool(e2e_equal)},
         "token_reordering": reorder_info,
         "block_selectors_on_aligned_workload": selectors,
         "gpu_launches": headline_launches,

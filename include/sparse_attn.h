@@ -106,17 +106,27 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
                     const sparse_attn_params* params, int mode, int64_t* stats_out);
 
 /*
- * Same operation with HOST buffers (pinned for full speed; pageable works, without overlap): takes
- * device scratch from the stream-ordered pool, cuts the B*H heads (independent units) into up to 8
- * chunks and pipelines them over internal streams -- the host->device copy of chunk c+1 and the
- * device->host copy of chunk c-1 run under the kernel of chunk c -- then synchronises and frees.
+ * Same operation with HOST buffers (pinned for full speed; pageable works, without overlap): cuts
+ * the B*H heads (independent units) into up to 20 chunks and pipelines them over four internal
+ * streams -- the host->device copy of chunk c+1 and the device->host copy of chunk c-1 run under the
+ * kernel of chunk c, consecutive kernels alternate between two streams -- then synchronises.
  * params->skip_mask_out / margin_out / skip_mask_in, if set, are host pointers here too; work is
  * ordered after whatever is already enqueued on params->stream.  Used for end-to-end timing;
  * layouts as above.  Synchronous: on return every output buffer is complete.
+ * Memory: the device copies of q, k, v, out (and of the optional buffers) come from a stream-ordered
+ * memory pool that belongs to this library (one per device; the device's default pool and its
+ * attributes are never touched).  Freed scratch STAYS in that pool for the next call -- after a
+ * config-3-sized call about 4 GB -- until sparse_attn_release_scratch() returns it to the driver.
+ * The internal streams and events are recycled across calls in the same way.
  */
 int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse,
                          int B, int H, int N, int D,
                          const sparse_attn_params* params, int mode, int64_t* stats_out);
+
+/* Returns the memory that sparse_attn_fwd_host keeps in the library's scratch pool of the CURRENT device to the
+ * driver (cudaMemPoolTrimTo 0) and destroys that device's recycled internal streams / events.  Call it when no
+ * sparse_attn_fwd_host call is running on the device; the next such call simply allocates again. */
+int sparse_attn_release_scratch(void);
 
 /* lambda = ln((1 - recall) / N): the worst-case threshold under which every row keeps more than
  * `recall` of its softmax mass (lambda = ln(eps / L)).  Pure host function. */

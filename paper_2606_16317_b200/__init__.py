@@ -27,6 +27,7 @@ from .binding import (  # noqa: F401
     sparse_attn_reorder_tokens,
     sparse_attn_output_error,
     sparse_attn_recall_stats,
+    sparse_attn_release_scratch,
     sparse_attn_row_topk_curve,
     sparse_attn_row_topk_curve_static,
     sparse_attn_select_blocks,

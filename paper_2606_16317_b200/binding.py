@@ -22,6 +22,7 @@ _lib = None
 EXPORTED_SYMBOLS = (
     "sparse_attn_fwd",
     "sparse_attn_fwd_host",
+    "sparse_attn_release_scratch",
     "sparse_attn_lambda_from_recall",
     "sparse_attn_lambda_from_preal",
     "sparse_attn_block_mass",
@@ -81,6 +82,8 @@ def _load():
         lib.sparse_attn_fwd.argtypes = fwd_args
         lib.sparse_attn_fwd_host.restype = ctypes.c_int
         lib.sparse_attn_fwd_host.argtypes = fwd_args
+        lib.sparse_attn_release_scratch.restype = ctypes.c_int
+        lib.sparse_attn_release_scratch.argtypes = []
         lib.sparse_attn_lambda_from_recall.restype = ctypes.c_double
         lib.sparse_attn_lambda_from_recall.argtypes = [ctypes.c_double, ctypes.c_int]
         lib.sparse_attn_lambda_from_preal.restype = ctypes.c_double
@@ -132,6 +135,15 @@ def status_string(status: int) -> str:
 
 def last_error() -> str:
     return _load().sparse_attn_last_error().decode()
+
+
+def sparse_attn_release_scratch() -> int:
+    """C entry point `sparse_attn_release_scratch`: hand the scratch `sparse_attn_fwd_host` retains on the current device
+    back to the driver."""
+    rc = _load().sparse_attn_release_scratch()
+    if rc != 0:
+        raise SparseAttnError(rc, last_error())
+    return rc
 
 
 def lambda_from_recall(recall: float, N: int) -> float:

@@ -308,6 +308,14 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             };
             if (!kSparse) {
                 for (int j = 0; j < T_c; ++j) load_v(j);
+            } else if (kMass) {
+                // block-mass kernel: every tile is voted skipped and V is never read -- no V traffic at all, every
+                // v_full phase is completed with a plain arrive (the issuers still pace the ring through v_empty)
+                for (int j = 0; j < T_c; ++j) {
+                    wait_slot_free(j);
+                    if (lane == 0) mbar_arrive(v_full(j % NV));
+                    __syncwarp();
+                }
             } else {
                 // Sparse modes: V_j is needed iff some slot keeps tile j.  This warp reads the votes of both slots
                 // (barrier dec), fetches V_j if it is needed and not yet there, and after a kept tile fetches V_{j+1}
@@ -346,14 +354,13 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
             }
         } else if (warp == kMmaWarp0 || warp == kMmaWarp1) {
             // ========================================================== MMA issuer(s) (a2, a6)
-            // kIssuers == 2: warp 9 drives slot 0 and warp 11 slot 1 (every mode; measured on config 1: DENSE 10.16 ms with
+            // Two issuers: warp 9 drives slot 0 and warp 11 slot 1 (every mode; measured on config 1: DENSE 10.16 ms with
             // two issuers and the gate below against 10.32 ms with one issuer driving both slots in turn; without the
-            // gate 11.8 ms).  The single-issuer path (kIssuers == 1, warp 11 idle) is kept for comparison.
-            constexpr int kIssuers = 2;
-            constexpr bool kGate = kIssuers == 2;
-            const int x_lo = (kIssuers == 2 && warp == kMmaWarp1) ? 1 : 0;
-            const int x_hi = (kIssuers == 2) ? x_lo + 1 : nX;        // this warp drives slots [x_lo, x_hi)
-            if ((kIssuers == 2 || warp == kMmaWarp0) && x_lo < nX) {
+            // gate 11.8 ms -- DESIGN.md section 9).
+            constexpr bool kGate = true;
+            const int x_lo = (warp == kMmaWarp1) ? 1 : 0;
+            const int x_hi = x_lo + 1;                               // this warp drives slots [x_lo, x_hi)
+            if (x_lo < nX) {
             auto issue_qk = [&](int x, uint32_t kaddr) {             // S_x = Q_x K^T, one N = BC instruction per k step
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {

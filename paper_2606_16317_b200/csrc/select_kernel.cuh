@@ -49,7 +49,9 @@ select_blocks_greedy_kernel(const float* __restrict__ mass, const float* __restr
     extern __shared__ float rowbuf[];
     float* row = rowbuf;
     float* rsq = rowbuf + T_c;
-    __shared__ int first_violation;
+    // rank of the first tile whose removal would violate Eq. 3; it lives in the rank slot of tile 0, which is never a
+    // candidate, so that the kernel's shared memory is exactly 3 T_c floats (48 KB at T_c = kSelectMaxTc, the default limit)
+    int& first_violation = *reinterpret_cast<int*>(rowbuf + 2 * T_c);
     const size_t base = (static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * static_cast<size_t>(T_c);
     for (int j = threadIdx.x; j < T_c; j += blockDim.x) { row[j] = mass[base + j]; rsq[j] = sqmass[base + j]; }
     if (threadIdx.x == 0) first_violation = T_c;

@@ -9,6 +9,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
+#include <vector>
 
 #include "fwd_kernel.cuh"
 #include "reorder_kernel.cuh"
@@ -46,15 +48,17 @@ using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 int get_encode_fn(EncodeTiledFn* out) {
+    static std::once_flag once;
     static EncodeTiledFn cached = nullptr;
-    if (!cached) {
+    static cudaError_t first_err = cudaSuccess;
+    std::call_once(once, [] {
         void* fn = nullptr;
         cudaDriverEntryPointQueryResult qres;
-        CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
-        if (qres != cudaDriverEntryPointSuccess || !fn)
-            return fail(SPARSE_ATTN_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available");
-        cached = reinterpret_cast<EncodeTiledFn>(fn);
-    }
+        first_err = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (first_err == cudaSuccess && qres == cudaDriverEntryPointSuccess) cached = reinterpret_cast<EncodeTiledFn>(fn);
+    });
+    if (!cached)
+        return fail(SPARSE_ATTN_ERR_CUDA, "cuTensorMapEncodeTiled entry point not available (%s)", cudaGetErrorString(first_err));
     *out = cached;
     return 0;
 }
@@ -165,6 +169,95 @@ int check_device() {
     return 0;
 }
 
+int sm_count(int* n_sm) {                                    // per call: the current device may differ between calls
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    CUDA_TRY(cudaDeviceGetAttribute(n_sm, cudaDevAttrMultiProcessorCount, dev));
+    return 0;
+}
+
+// ---- device scratch of sparse_attn_fwd_host: a pool of the library's own, one per device, so that neither the release
+// threshold nor the retained memory touches the device's default pool (which the host application may be using).
+constexpr int kMaxPoolDevices = 64;
+std::mutex g_host_mu;
+cudaMemPool_t g_scratch_pool[kMaxPoolDevices] = {};
+
+int scratch_pool(int dev, cudaMemPool_t* pool) {
+    if (dev < 0 || dev >= kMaxPoolDevices) return fail(SPARSE_ATTN_ERR_DEVICE, "device ordinal %d outside [0, %d)", dev, kMaxPoolDevices);
+    std::lock_guard<std::mutex> lock(g_host_mu);
+    if (!g_scratch_pool[dev]) {
+        cudaMemPoolProps props;
+        std::memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t created = nullptr;
+        CUDA_TRY(cudaMemPoolCreate(&created, &props));
+        uint64_t keep = UINT64_MAX;                          // freed scratch stays in THIS pool until sparse_attn_release_scratch
+        cudaError_t err = cudaMemPoolSetAttribute(created, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (err != cudaSuccess) {
+            cudaMemPoolDestroy(created);
+            return fail(SPARSE_ATTN_ERR_CUDA, "cudaMemPoolSetAttribute failed: %s", cudaGetErrorString(err));
+        }
+        g_scratch_pool[dev] = created;
+    }
+    *pool = g_scratch_pool[dev];
+    return 0;
+}
+
+// ---- the internal streams and events of one sparse_attn_fwd_host call; sets are recycled across calls (a call takes a
+// free set of its device or creates one, and hands it back), so that a steady caller creates them once.
+constexpr int kMaxChunks = 20;      // (config 3: 2 heads = 4 whole waves per chunk; 8 chunks left 3 ms of copy head and tail exposed)
+struct HostSet {
+    int dev = -1;
+    cudaStream_t s_in = nullptr, s_out = nullptr, s_k[2] = {nullptr, nullptr};
+    cudaEvent_t ev_start = nullptr, ev_in[kMaxChunks] = {}, ev_done[kMaxChunks] = {}, ev_end[4] = {};
+};
+std::vector<HostSet*> g_host_sets;                           // free sets, any device (guarded by g_host_mu)
+
+void destroy_host_set(HostSet* h) {
+    for (cudaStream_t s : {h->s_in, h->s_out, h->s_k[0], h->s_k[1]}) if (s) cudaStreamDestroy(s);
+    if (h->ev_start) cudaEventDestroy(h->ev_start);
+    for (int c = 0; c < kMaxChunks; ++c) { if (h->ev_in[c]) cudaEventDestroy(h->ev_in[c]); if (h->ev_done[c]) cudaEventDestroy(h->ev_done[c]); }
+    for (cudaEvent_t e : h->ev_end) if (e) cudaEventDestroy(e);
+    delete h;
+}
+
+int acquire_host_set(int dev, HostSet** out) {
+    {
+        std::lock_guard<std::mutex> lock(g_host_mu);
+        for (size_t i = 0; i < g_host_sets.size(); ++i)
+            if (g_host_sets[i]->dev == dev) {
+                *out = g_host_sets[i];
+                g_host_sets.erase(g_host_sets.begin() + i);
+                return 0;
+            }
+    }
+    HostSet* h = new HostSet;
+    h->dev = dev;
+    cudaError_t err = cudaSuccess;
+    auto ok = [&](cudaError_t e) { if (err == cudaSuccess) err = e; return err == cudaSuccess; };
+    for (cudaStream_t* s : {&h->s_in, &h->s_out, &h->s_k[0], &h->s_k[1]}) ok(cudaStreamCreateWithFlags(s, cudaStreamNonBlocking));
+    ok(cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming));
+    for (int c = 0; c < kMaxChunks; ++c) {
+        ok(cudaEventCreateWithFlags(&h->ev_in[c], cudaEventDisableTiming));
+        ok(cudaEventCreateWithFlags(&h->ev_done[c], cudaEventDisableTiming));
+    }
+    for (cudaEvent_t& e : h->ev_end) ok(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    if (err != cudaSuccess) {
+        destroy_host_set(h);
+        return fail(SPARSE_ATTN_ERR_CUDA, "creating the internal streams / events failed: %s", cudaGetErrorString(err));
+    }
+    *out = h;
+    return 0;
+}
+
+void release_host_set(HostSet* h) {
+    std::lock_guard<std::mutex> lock(g_host_mu);
+    g_host_sets.push_back(h);
+}
+
 }  // namespace
 
 extern "C" {
@@ -228,10 +321,12 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     return launch<64, 64, 2, 3, 2, true, true>(tq, tk, tv, a, BH, r.stream);
 }
 
-// Host-buffer entry: the B*H heads are independent units, so they are cut into chunks and pipelined over three
-// streams -- H2D of chunk c+1 and D2H of chunk c-1 run under the kernel of chunk c (PCIe is full duplex), and the
-// kernels of consecutive chunks alternate between two streams so that the next chunk's CTAs fill the last wave of the
-// previous one.  Device scratch comes from the stream-ordered pool (one allocation per tensor and call).
+// Host-buffer entry: the B*H heads are independent units, so they are cut into chunks and pipelined over four internal
+// streams -- H2D of chunk c+1 (s_in) and D2H of chunk c-1 (s_out) run under the kernel of chunk c (PCIe is full duplex),
+// and the kernels of consecutive chunks alternate between two streams (s_k[0..1]) so that the next chunk's CTAs fill the
+// last wave of the previous one.  Device scratch comes from the library's own stream-ordered pool (one allocation per
+// tensor and call; freed memory stays in that pool until sparse_attn_release_scratch); the streams and events are
+// recycled across calls.
 int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out, float* lse, int B, int H, int N, int D,
                          const sparse_attn_params* params, int mode, int64_t* stats_out) {
     Resolved r;
@@ -242,11 +337,14 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     const size_t head_elems = static_cast<size_t>(N) * D;
     const size_t T_r = (N + r.tile_q - 1) / r.tile_q, T_c = (N + r.tile_k - 1) / r.tile_k;
     const size_t head_tiles = T_r * T_c;
-    constexpr int kMaxChunks = 20;      // (config 3: 2 heads = 4 whole waves per chunk; 8 chunks left 3 ms of copy head and tail exposed)
     const int n_chunks = static_cast<int>(std::min<size_t>(BH, kMaxChunks));
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    cudaMemPool_t pool = nullptr;
+    if ((rc = scratch_pool(dev, &pool))) return rc;
+    HostSet* hs = nullptr;
+    if ((rc = acquire_host_set(dev, &hs))) return rc;
     cudaStream_t st = r.stream;
-    cudaStream_t s_in = nullptr, s_out = nullptr, s_k[2] = {nullptr, nullptr};
-    cudaEvent_t ev_start = nullptr, ev_in[kMaxChunks] = {}, ev_done[kMaxChunks] = {}, ev_end[4] = {};
     void *dq = nullptr, *dk = nullptr, *dv = nullptr, *dout = nullptr;
     float *dlse = nullptr, *dmargin = nullptr;
     int64_t* dstats = nullptr;
@@ -255,10 +353,7 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
         void* bufs[] = {dq, dk, dv, dout, dlse, dstats, dmask, dmargin, dmask_in};
         for (void* b : bufs) if (b) cudaFreeAsync(b, st);
         cudaStreamSynchronize(st);
-        for (cudaStream_t s : {s_in, s_out, s_k[0], s_k[1]}) if (s) cudaStreamDestroy(s);
-        if (ev_start) cudaEventDestroy(ev_start);
-        for (int c = 0; c < kMaxChunks; ++c) { if (ev_in[c]) cudaEventDestroy(ev_in[c]); if (ev_done[c]) cudaEventDestroy(ev_done[c]); }
-        for (cudaEvent_t e : ev_end) if (e) cudaEventDestroy(e);
+        release_host_set(hs);
     };
 #define HOST_TRY(expr)                                                                                   \
     do {                                                                                                 \
@@ -269,36 +364,19 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
             return fail(SPARSE_ATTN_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(err__));        \
         }                                                                                                \
     } while (0)
-    {                            // keep freed scratch in the pool between calls instead of returning it to the driver
-        int dev = 0;
-        cudaMemPool_t pool;
-        HOST_TRY(cudaGetDevice(&dev));
-        HOST_TRY(cudaDeviceGetDefaultMemPool(&pool, dev));
-        uint64_t keep = UINT64_MAX;
-        HOST_TRY(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-    }
-    HOST_TRY(cudaMallocAsync(&dq, BH * head_elems * 2, st));
-    HOST_TRY(cudaMallocAsync(&dk, BH * head_elems * 2, st));
-    HOST_TRY(cudaMallocAsync(&dv, BH * head_elems * 2, st));
-    HOST_TRY(cudaMallocAsync(&dout, BH * head_elems * 2, st));
-    if (lse) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dlse), BH * N * sizeof(float), st));
-    if (stats_out) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dstats), BH * 2 * sizeof(int64_t), st));
-    if (r.skip_mask) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dmask), BH * head_tiles, st));
-    if (r.margin) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dmargin), BH * head_tiles * sizeof(float), st));
-    if (r.mask_in) HOST_TRY(cudaMallocAsync(reinterpret_cast<void**>(&dmask_in), BH * head_tiles, st));
-    HOST_TRY(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
-    HOST_TRY(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
-    HOST_TRY(cudaStreamCreateWithFlags(&s_k[0], cudaStreamNonBlocking));
-    HOST_TRY(cudaStreamCreateWithFlags(&s_k[1], cudaStreamNonBlocking));
-    HOST_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
-    for (int c = 0; c < n_chunks; ++c) {
-        HOST_TRY(cudaEventCreateWithFlags(&ev_in[c], cudaEventDisableTiming));
-        HOST_TRY(cudaEventCreateWithFlags(&ev_done[c], cudaEventDisableTiming));
-    }
-    for (cudaEvent_t& e : ev_end) HOST_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    HOST_TRY(cudaMallocFromPoolAsync(&dq, BH * head_elems * 2, pool, st));
+    HOST_TRY(cudaMallocFromPoolAsync(&dk, BH * head_elems * 2, pool, st));
+    HOST_TRY(cudaMallocFromPoolAsync(&dv, BH * head_elems * 2, pool, st));
+    HOST_TRY(cudaMallocFromPoolAsync(&dout, BH * head_elems * 2, pool, st));
+    if (lse) HOST_TRY(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&dlse), BH * N * sizeof(float), pool, st));
+    if (stats_out) HOST_TRY(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&dstats), BH * 2 * sizeof(int64_t), pool, st));
+    if (r.skip_mask) HOST_TRY(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&dmask), BH * head_tiles, pool, st));
+    if (r.margin) HOST_TRY(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&dmargin), BH * head_tiles * sizeof(float), pool, st));
+    if (r.mask_in) HOST_TRY(cudaMallocFromPoolAsync(reinterpret_cast<void**>(&dmask_in), BH * head_tiles, pool, st));
+    cudaStream_t s_in = hs->s_in, s_out = hs->s_out, s_k[2] = {hs->s_k[0], hs->s_k[1]};
     // the scratch allocations (and whatever the caller enqueued before) are ordered on `st`
-    HOST_TRY(cudaEventRecord(ev_start, st));
-    for (cudaStream_t s : {s_in, s_out, s_k[0], s_k[1]}) HOST_TRY(cudaStreamWaitEvent(s, ev_start, 0));
+    HOST_TRY(cudaEventRecord(hs->ev_start, st));
+    for (cudaStream_t s : {s_in, s_out, s_k[0], s_k[1]}) HOST_TRY(cudaStreamWaitEvent(s, hs->ev_start, 0));
 
     sparse_attn_params dp;
     std::memset(&dp, 0, sizeof dp);
@@ -315,9 +393,9 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
         HOST_TRY(cudaMemcpyAsync(atw(dq, eoff), at(q, eoff), ebytes, cudaMemcpyHostToDevice, s_in));
         HOST_TRY(cudaMemcpyAsync(atw(dk, eoff), at(k, eoff), ebytes, cudaMemcpyHostToDevice, s_in));
         HOST_TRY(cudaMemcpyAsync(atw(dv, eoff), at(v, eoff), ebytes, cudaMemcpyHostToDevice, s_in));
-        HOST_TRY(cudaEventRecord(ev_in[c], s_in));
+        HOST_TRY(cudaEventRecord(hs->ev_in[c], s_in));
         cudaStream_t sk = s_k[c & 1];
-        HOST_TRY(cudaStreamWaitEvent(sk, ev_in[c], 0));
+        HOST_TRY(cudaStreamWaitEvent(sk, hs->ev_in[c], 0));
         dp.stream = sk;
         dp.skip_mask_out = dmask ? dmask + h0 * head_tiles : nullptr;
         dp.margin_out = dmargin ? dmargin + h0 * head_tiles : nullptr;
@@ -325,8 +403,8 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
         rc = sparse_attn_fwd(atw(dq, eoff), atw(dk, eoff), atw(dv, eoff), atw(dout, eoff), dlse ? dlse + h0 * N : nullptr, 1,
                              static_cast<int>(nh), N, D, &dp, mode, dstats ? dstats + h0 * 2 : nullptr);
         if (rc) { cudaDeviceSynchronize(); cleanup(); return rc; }
-        HOST_TRY(cudaEventRecord(ev_done[c], sk));
-        HOST_TRY(cudaStreamWaitEvent(s_out, ev_done[c], 0));
+        HOST_TRY(cudaEventRecord(hs->ev_done[c], sk));
+        HOST_TRY(cudaStreamWaitEvent(s_out, hs->ev_done[c], 0));
         HOST_TRY(cudaMemcpyAsync(atw(out, eoff), at(dout, eoff), ebytes, cudaMemcpyDeviceToHost, s_out));
         if (lse) HOST_TRY(cudaMemcpyAsync(lse + h0 * N, dlse + h0 * N, nh * N * sizeof(float), cudaMemcpyDeviceToHost, s_out));
         if (stats_out) HOST_TRY(cudaMemcpyAsync(stats_out + h0 * 2, dstats + h0 * 2, nh * 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, s_out));
@@ -337,12 +415,32 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     // join everything back into `st`, then wait: the call is synchronous
     cudaStream_t joins[4] = {s_in, s_out, s_k[0], s_k[1]};
     for (int i = 0; i < 4; ++i) {
-        HOST_TRY(cudaEventRecord(ev_end[i], joins[i]));
-        HOST_TRY(cudaStreamWaitEvent(st, ev_end[i], 0));
+        HOST_TRY(cudaEventRecord(hs->ev_end[i], joins[i]));
+        HOST_TRY(cudaStreamWaitEvent(st, hs->ev_end[i], 0));
     }
     HOST_TRY(cudaStreamSynchronize(st));
     cleanup();
 #undef HOST_TRY
+    return 0;
+}
+
+// Hands the memory sparse_attn_fwd_host keeps in the library's scratch pool of the current device back to the driver,
+// and drops the recycled stream / event sets of that device.
+int sparse_attn_release_scratch(void) {
+    g_last_error[0] = '\0';
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    std::vector<HostSet*> mine;
+    cudaMemPool_t pool = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_host_mu);
+        for (size_t i = 0; i < g_host_sets.size();)
+            if (g_host_sets[i]->dev == dev) { mine.push_back(g_host_sets[i]); g_host_sets.erase(g_host_sets.begin() + i); }
+            else ++i;
+        if (dev >= 0 && dev < kMaxPoolDevices) pool = g_scratch_pool[dev];
+    }
+    for (HostSet* h : mine) destroy_host_set(h);
+    if (pool) CUDA_TRY(cudaMemPoolTrimTo(pool, 0));
     return 0;
 }
 
@@ -382,7 +480,8 @@ int sparse_attn_block_stats(const void* q, const void* k, const float* lse, floa
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     CUDA_TRY(cudaMemsetAsync(mass_out, 0, sizeof(float) * static_cast<size_t>(BH) * a.T_r * a.T_c, st));
     if (sqmass_out) CUDA_TRY(cudaMemsetAsync(sqmass_out, 0, sizeof(float) * static_cast<size_t>(BH) * a.T_r * a.T_c, st));
-    // V is never read for P V in this mode (every tile is voted skipped); the V map aliases K for the one prefetch of tile 0
+    // V is never read in this mode (every tile is voted skipped and the V warp fetches nothing); the V map aliases K only
+    // because the kernel's signature wants one
     if (D == 128) return launch<128, 128, 1, DSA_NK, DSA_NV, true, false, 0>(tq, tk, tk, a, BH, st);
     return launch<64, 64, 2, 3, 2, true, false, 0>(tq, tk, tk, a, BH, st);
 }
@@ -466,9 +565,8 @@ int sparse_attn_reorder_tokens(const void* src, void* dst, int B, int H, int N, 
     if (s0 < d0 + bytes && d0 < s0 + bytes) return fail(SPARSE_ATTN_ERR_PARAMS, "src and dst overlap");
     int rc = check_device();
     if (rc) return rc;
-    int n_sm = 0, dev = 0;                                   // per call: the current device may differ between calls
-    CUDA_TRY(cudaGetDevice(&dev));
-    CUDA_TRY(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    int n_sm = 0;
+    if ((rc = sm_count(&n_sm))) return rc;
     const long long rows = static_cast<long long>(B) * H * N;
     const int lanes = D / 8;                                 // 16 bytes per thread
     const long long blocks_needed = (rows + (256 / lanes) * 4 - 1) / ((256 / lanes) * 4);
@@ -490,8 +588,10 @@ int sparse_attn_recall_stats(const float* lse_retained, const float* lse_dense, 
     int rc = check_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int n_sm = 0;
+    if ((rc = sm_count(&n_sm))) return rc;
+    const int grid = static_cast<int>(std::min<int64_t>((n_rows + 255) / 256, static_cast<int64_t>(n_sm) * 8));   // 8 CTAs of 256 threads per SM
     dsa::stats_init_kernel<<<1, 1, 0, st>>>(stats_out, INFINITY, 0.0);
-    const int grid = static_cast<int>(std::min<int64_t>((n_rows + 255) / 256, 148 * 8));   // (8 CTAs per B200 SM)
     dsa::recall_stats_kernel<<<grid, 256, 0, st>>>(lse_retained, lse_dense, n_rows, stats_out);
     CUDA_TRY(cudaGetLastError());
     g_reorder_launches.fetch_add(2);
@@ -507,9 +607,11 @@ int sparse_attn_output_error(const void* out_a, const void* out_b, int64_t n_ele
     int rc = check_device();
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    dsa::stats_init_kernel<<<1, 1, 0, st>>>(stats_out, 0.0, 0.0);
     const int64_t n2 = n_elems / 2;
-    const int grid = static_cast<int>(std::min<int64_t>((n2 + 255) / 256, 148 * 8));
+    int n_sm = 0;
+    if ((rc = sm_count(&n_sm))) return rc;
+    const int grid = static_cast<int>(std::min<int64_t>((n2 + 255) / 256, static_cast<int64_t>(n_sm) * 8));
+    dsa::stats_init_kernel<<<1, 1, 0, st>>>(stats_out, 0.0, 0.0);
     dsa::output_error_kernel<<<grid, 256, 0, st>>>(static_cast<const __nv_bfloat162*>(out_a), static_cast<const __nv_bfloat162*>(out_b), n2, stats_out);
     CUDA_TRY(cudaGetLastError());
     g_reorder_launches.fetch_add(2);
@@ -542,12 +644,26 @@ int sparse_attn_row_topk_curve(const void* q, const void* k, const void* v, int 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int32_t *d_rows = nullptr, *d_keep = nullptr;
     float* scratch = nullptr;
-    CUDA_TRY(cudaMallocAsync(reinterpret_cast<void**>(&d_rows), sizeof(int32_t) * 2 * n_rows, st));
-    CUDA_TRY(cudaMallocAsync(reinterpret_cast<void**>(&d_keep), sizeof(int32_t) * n_keep, st));
-    CUDA_TRY(cudaMallocAsync(reinterpret_cast<void**>(&scratch), sizeof(float) * static_cast<size_t>(n_rows) * N, st));
-    CUDA_TRY(cudaMemcpyAsync(d_rows, rows, sizeof(int32_t) * 2 * n_rows, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(d_keep, keep_counts, sizeof(int32_t) * n_keep, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaStreamSynchronize(st));                     // rows / keep_counts may be pageable: the caller may reuse them now
+    auto release = [&]() {                                   // stream-ordered: safe whether or not the kernel was enqueued
+        cudaError_t first = cudaSuccess;
+        for (void* b : {static_cast<void*>(scratch), static_cast<void*>(d_keep), static_cast<void*>(d_rows)})
+            if (b) { cudaError_t e = cudaFreeAsync(b, st); if (first == cudaSuccess) first = e; }
+        return first;
+    };
+#define CURVE_TRY(expr)                                                                                  \
+    do {                                                                                                 \
+        cudaError_t err__ = (expr);                                                                      \
+        if (err__ != cudaSuccess) {                                                                      \
+            release();                                                                                   \
+            return fail(SPARSE_ATTN_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(err__));        \
+        }                                                                                                \
+    } while (0)
+    CURVE_TRY(cudaMallocAsync(reinterpret_cast<void**>(&d_rows), sizeof(int32_t) * 2 * n_rows, st));
+    CURVE_TRY(cudaMallocAsync(reinterpret_cast<void**>(&d_keep), sizeof(int32_t) * n_keep, st));
+    CURVE_TRY(cudaMallocAsync(reinterpret_cast<void**>(&scratch), sizeof(float) * static_cast<size_t>(n_rows) * N, st));
+    CURVE_TRY(cudaMemcpyAsync(d_rows, rows, sizeof(int32_t) * 2 * n_rows, cudaMemcpyHostToDevice, st));
+    CURVE_TRY(cudaMemcpyAsync(d_keep, keep_counts, sizeof(int32_t) * n_keep, cudaMemcpyHostToDevice, st));
+    CURVE_TRY(cudaStreamSynchronize(st));                    // rows / keep_counts may be pageable: the caller may reuse them now
     const float scale = softmax_scale > 0.f ? softmax_scale : 1.0f / std::sqrt(static_cast<float>(D));
     auto qp = static_cast<const __nv_bfloat16*>(q), kp = static_cast<const __nv_bfloat16*>(k), vp = static_cast<const __nv_bfloat16*>(v);
     if (D == 128)
@@ -556,11 +672,10 @@ int sparse_attn_row_topk_curve(const void* q, const void* k, const void* v, int 
     else
         dsa::row_topk_curve_kernel<64><<<n_rows, dsa::kRowCurveThreads, 0, st>>>(qp, kp, vp, N, scale, d_rows, d_keep, n_keep, scratch,
                                                                                  kurtosis_out, recall_out, mae_out);
-    CUDA_TRY(cudaGetLastError());
+    CURVE_TRY(cudaGetLastError());
+#undef CURVE_TRY
     g_reorder_launches.fetch_add(1);
-    CUDA_TRY(cudaFreeAsync(scratch, st));
-    CUDA_TRY(cudaFreeAsync(d_keep, st));
-    CUDA_TRY(cudaFreeAsync(d_rows, st));
+    CUDA_TRY(release());
     return 0;
 }
 

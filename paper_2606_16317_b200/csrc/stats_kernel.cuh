@@ -16,30 +16,34 @@ __global__ void stats_init_kernel(double* out, double v0, double v1) {
     out[1] = v1;
 }
 
-// positive doubles order like their bit patterns: atomicMin / atomicMax on the 64-bit integer view
-__device__ __forceinline__ void atomic_min_pos(double* addr, double v) {
-    atomicMin(reinterpret_cast<unsigned long long*>(addr), static_cast<unsigned long long>(__double_as_longlong(v)));
+// positive doubles order like their bit patterns: atomicMin / atomicMax on the 64-bit integer view.
+// In the minimum a NaN beats everything (a broken run must not report a healthy minimum): positive doubles also order
+// like SIGNED 64-bit integers, and a NaN with its sign bit set is below all of them
+__device__ __forceinline__ void atomic_min_pos_or_nan(double* addr, double v) {
+    const long long bits = (v != v) ? static_cast<long long>(0xfff8000000000000ull) : __double_as_longlong(v);
+    atomicMin(reinterpret_cast<long long*>(addr), bits);
 }
+__device__ __forceinline__ double min_or_nan(double a, double b) { return (a != a || b != b) ? NAN : fmin(a, b); }
 __device__ __forceinline__ void atomic_max_pos(double* addr, double v) {
     atomicMax(reinterpret_cast<unsigned long long*>(addr), static_cast<unsigned long long>(__double_as_longlong(v)));
 }
 
-// out[0] = min_r recall_r, out[1] = sum_r recall_r   (out pre-set to {+inf, 0})
+// out[0] = min_r recall_r (NaN if any row's recall is NaN), out[1] = sum_r recall_r   (out pre-set to {+inf, 0})
 __global__ void __launch_bounds__(256)
 recall_stats_kernel(const float* __restrict__ lse_retained, const float* __restrict__ lse_dense, long long n, double* out) {
     double mn = INFINITY, sm = 0.0;
     for (long long i = blockIdx.x * 256ll + threadIdx.x; i < n; i += static_cast<long long>(gridDim.x) * 256) {
         const double rec = exp(static_cast<double>(lse_retained[i]) - static_cast<double>(lse_dense[i]));
-        mn = fmin(mn, rec);
+        mn = min_or_nan(mn, rec);
         sm += rec;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+        mn = min_or_nan(mn, __shfl_xor_sync(0xffffffffu, mn, o));
         sm += __shfl_xor_sync(0xffffffffu, sm, o);
     }
     if ((threadIdx.x & 31) == 0) {
-        atomic_min_pos(out, mn);
+        atomic_min_pos_or_nan(out, mn);
         atomicAdd(out + 1, sm);
     }
 }

@@ -201,3 +201,36 @@ def test_mask_comparison_meets_the_target_and_fixed_depends_on_the_position_of_t
     gap_fixed = sp["flat_max_first", "fixed"] - sp["flat_max_last", "fixed"]
     gap_dyn = sp["flat_max_first", "dynamic"] - sp["flat_max_last", "dynamic"]
     assert gap_fixed > 0.5 and abs(gap_dyn) < gap_fixed
+
+
+@pytest.mark.gpu
+def test_recall_stats_reductions_and_nan_propagation():
+    """sparse_attn_recall_stats: {min, sum} of e^(lse_retained - lse_dense) against NumPy, on more rows than one grid pass
+    covers; a NaN row (a broken sparse run) must surface in the minimum instead of being dropped by fmin."""
+    import torch
+
+    import paper_2606_16317_b200 as sa
+    rng = np.random.default_rng(13)
+    n = 700_001
+    dense = rng.normal(5.0, 2.0, size=n).astype(np.float32)
+    kept = (dense + np.log(rng.uniform(0.2, 1.0, size=n))).astype(np.float32)
+    rec = np.exp(kept.astype(np.float64) - dense.astype(np.float64))
+    d_dense, d_kept = torch.from_numpy(dense).cuda(), torch.from_numpy(kept).cuda()
+    out = torch.full((2,), -7.0, device="cuda", dtype=torch.float64)
+    sa.sparse_attn_recall_stats(d_kept, d_dense, n, out)
+    torch.cuda.synchronize()
+    mn, sm = out.cpu().numpy()
+    assert mn == rec.min() and sm == pytest.approx(rec.sum(), rel=1e-12)
+    d_kept[123_456] = float("nan")
+    sa.sparse_attn_recall_stats(d_kept, d_dense, n, out)
+    torch.cuda.synchronize()
+    mn, sm = out.cpu().numpy()
+    assert math.isnan(mn) and math.isnan(sm)
+    # the output-error reduction beside it
+    a = torch.from_numpy(rng.standard_normal(100_000).astype(np.float32)).cuda().to(torch.bfloat16)
+    b = torch.from_numpy(rng.standard_normal(100_000).astype(np.float32)).cuda().to(torch.bfloat16)
+    sa.sparse_attn_output_error(a, b, a.numel(), out)
+    torch.cuda.synchronize()
+    diff = np.abs(a.float().cpu().numpy().astype(np.float64) - b.float().cpu().numpy().astype(np.float64))
+    mx, sm = out.cpu().numpy()
+    assert mx == diff.max() and sm == pytest.approx(diff.sum(), rel=1e-12)

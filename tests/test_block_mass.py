@@ -231,3 +231,35 @@ def test_gpu_selectors_match_oracle_and_drive_mask_mode(seed):
         if kind == sa.SELECT_TOPP:                          # row recall >= share of the row's own tile masses kept: sanity
             rec = torch.exp(lse_m - lse)
             assert float(rec.mean()) > param - 0.05
+
+
+@pytest.mark.gpu
+def test_gpu_selectors_at_the_documented_maximum_row_length(seed):
+    """T_c = 4096 is the largest row of tiles the selectors accept; the greedy kernel then needs exactly 48 KB of shared
+    memory (it used to need 4 bytes more than the default limit and failed to launch).  Random mass rows, one Q tile per
+    head, against the oracle's selections."""
+    import torch
+    T_c, tile = 4096, 128
+    N = tile                                                                    # T_r = 1 row of tiles per head
+    rng = np.random.default_rng([seed, 4096])
+    H = 3
+    p = rng.dirichlet(np.full(T_c, 0.3), size=(1, H, 1)).astype(np.float32)     # P_j of a row, sums to 1
+    mass = (p * tile).astype(np.float32)                                        # block sums over 128 rows
+    sq = (p ** 2 * tile * rng.uniform(0.5, 1.5, size=p.shape)).astype(np.float32)
+    dm, ds = torch.from_numpy(mass).cuda(), torch.from_numpy(sq).cuda()
+    bitmap = torch.full((1, H, 1, T_c), 255, device="cuda", dtype=torch.uint8)
+    for theta in (1e-7, 1e-5):
+        sa.sparse_attn_select_blocks_greedy(dm, ds, bitmap, 1, H, N, tile, T_c, theta)
+        torch.cuda.synchronize()
+        got = bitmap.cpu().numpy()
+        for h in range(H):
+            ref = oracle.select_greedy(mass[0, h].astype(np.float64), sq[0, h].astype(np.float64), N, tile, theta)
+            assert np.array_equal(got[0, h], ref), (theta, h, int(got[0, h].sum()), int(ref.sum()))
+        assert 0 < got.sum() < H * T_c
+    for kind, param in ((sa.SELECT_TOPK, 0.25), (sa.SELECT_TOPP, 0.9)):
+        sa.sparse_attn_select_blocks(dm, bitmap, 1, H, 1, T_c, kind, param)
+        torch.cuda.synchronize()
+        got = bitmap.cpu().numpy()
+        for h in range(H):
+            ref = (oracle.select_topk if kind == sa.SELECT_TOPK else oracle.select_topp)(mass[0, h].astype(np.float64), param)
+            assert np.array_equal(got[0, h], ref), (kind, h)
