@@ -186,7 +186,7 @@ def run_reference(args, cfg, lam):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT,
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": mean_s * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "mode": "dynamic", "lambda": lam, "step": res["sample"]},
+        "config": {"workload": workload_name(cfg_full), "mode": "dynamic", "lambda": lam, "step": res["sample"]},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": res["cores"], "kind": "oracle", "sample": res["sample"]},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -568,6 +568,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--preheat", type=float, default=1.5, help="seconds of untimed DENSE calls before each workload's timed modes")
     ap.add_argument("--modes", default="dense,fixed,dynamic", help="subset of modes to time (profiling runs)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own full batch (default, the driver's contract); strong = ONE batch, its heads "
+                         "sharded over the ranks (SURVEY.md 8(e)), each rank generating only its own heads")
     ap.add_argument("--report", default=None, choices=["cfg2", "cfg3", "cfg4", "masks", "kurtosis"],
                     help="run one of the sweeps BASELINE.json configs[2..4] / SURVEY.md NEXT-4 ask for and print it as JSON")
     args = ap.parse_args()
@@ -585,9 +588,23 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    # inputs first (spawned workers): weak scaling, every rank draws its own batch (different seed), same shape
     workers = max(1, host_workers() // max(1, min(world, 8)))
-    host_data = {args.config: make_qkv(cfg, args.seed + 1000 * rank, workers=workers)}
+    cfg_full = cfg
+    strong = args.scaling == "strong" and world > 1
+    if strong:
+        # strong scaling: ONE batch of cfg.H heads, rank r owns the contiguous range shard_heads(H, world, r) and draws
+        # only those heads (same seed on every rank: head h has the bits it has in the single-GPU run)
+        import dataclasses
+        from paper_2606_16317_b200.sharding import shard_heads
+        if world > cfg.H:
+            raise SystemExit(f"--scaling strong needs at most {cfg.H} ranks (one head per rank)")
+        h0, h1 = shard_heads(cfg.H, world, rank)
+        host_data = {args.config: make_qkv(cfg, args.seed, heads=range(h0, h1), workers=workers)}
+        cfg = dataclasses.replace(cfg, H=h1 - h0)            # the local problem: everything below sees its own heads only
+        args.no_aligned = True
+    else:
+        # inputs first (spawned workers): weak scaling, every rank draws its own batch (different seed), same shape
+        host_data = {args.config: make_qkv(cfg, args.seed + 1000 * rank, workers=workers)}
     aligned_name = args.config + "_aligned"
     if not args.no_aligned and aligned_name in CONFIGS:
         host_data[aligned_name] = make_qkv(CONFIGS[aligned_name], args.seed + 1000 * rank, workers=workers)
@@ -609,7 +626,8 @@ def main():
             dist.barrier()
 
     tb, ts, peak_kind = measured_peaks()
-    BH = cfg.B * cfg.H
+    BH = cfg.B * cfg.H                                       # heads of THIS rank
+    BH_total = cfg_full.B * cfg_full.H if strong else BH * world
     results = {}
     # (result key, generator config, brick of the token re-ordering or None)
     variants = [(args.config, args.config, None)]
@@ -624,7 +642,7 @@ def main():
     headline_launches = 0
     want = args.modes.split(",")
     for vi, (name, gen_name, brick) in enumerate(variants):
-        vcfg = CONFIGS[gen_name]
+        vcfg = cfg if gen_name == args.config else CONFIGS[gen_name]
         g = Gpu(sa, torch, vcfg, *host_data[gen_name], barrier=barrier)
         if brick is not None:
             reorder_info, (g.q, g.k, g.v) = time_reorder(sa, torch, vcfg, brick, (g.q, g.k, g.v), g.out, args.steps, args.warmup)
@@ -656,11 +674,12 @@ def main():
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
                 total = float(t.item())
                 from paper_2606_16317_b200.sharding import gather_stats
-                # every rank owns cfg.H heads of the (world * H)-head job: assemble the per-head counts
-                st_all = gather_stats(torch.from_numpy(st).cuda(), cfg.H * world).cpu().numpy()[None]
+                # weak: every rank owns cfg.H heads of the (world * H)-head job; strong: its shard of the H heads (sizes may
+                # differ by one) -- assemble the per-head counts in rank order
+                st_all = gather_stats(torch.from_numpy(st).cuda(), BH_total // cfg.B).cpu().numpy()[None]
             else:
                 st_all = st[None]
-            res[mname] = mode_entry(g, BH * world, total / args.steps, per, st_all, st[None])
+            res[mname] = mode_entry(g, BH_total, total / args.steps, per, st_all, st[None])
             if mname == "dense":
                 g.keep_dense()
             else:
@@ -771,12 +790,13 @@ def main():
         "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": head_total_ms / args.steps if world == 1 else main_res["ms"],
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-        "config": {"workload": workload_name(cfg), "mode": "dynamic", "lambda": lam,
+        "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": workload_name(cfg_full), "mode": "dynamic", "lambda": lam,
                    "lambda_rule": f"Eq. 7, P_real={P_REAL}",
                    "l2": "q+k+v+out = %.0f MB per step > 126 MB L2, no flush" % (4 * BH * cfg.N * cfg.D * 2 / 1e6),
                    "preheat_s": args.preheat,
-                   "parallelism": f"heads sharded, {world} rank(s), no data-path collective"},
+                   "parallelism": (f"one batch, its {cfg_full.H} heads sharded over {world} ranks, no data-path collective" if strong
+                                   else f"heads sharded, {world} rank(s) with one batch each, no data-path collective")},
         "sparsity_pct": 100.0 * main_res["sparsity"],
         "speedup_vs_dense": main_res["speedup_vs_dense"],
         "pct_tensor_peak_executed": {"dense": 100.0 * ach_dense / tb, "dynamic": 100.0 * ach_dyn / tb,
@@ -792,7 +812,7 @@ def main():
                      "dense_flop_per_launch": dense_res["executed_flop_per_launch_rank0"],
                      "dense_launch_ms": dense_res["kernel_ms_avg_rank0"]},
         "cpu_baseline": cpu_baseline,
-        "e2e": {"value": dense_flop(BH * world, cfg.N, cfg.D) / e2e_s / 1e12, "unit": UNIT,
+        "e2e": {"value": dense_flop(BH_total, cfg.N, cfg.D) / e2e_s / 1e12, "unit": UNIT,
                 "ms_per_step": e2e_s * 1e3, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "path": "sparse_attn_fwd_host: pinned host buffers, H2D + kernel + D2H pipelined over head chunks",
                 "equals_device_entry": bool(e2e_equal)},

@@ -1,4 +1,5 @@
-"""World-size-2 gloo test of the multi-GPU host logic (heads sharded, stats all-gathered)."""
+"""gloo tests (world size 2 and 3) of the multi-GPU host logic: heads sharded, stats all-gathered -- the code path of
+`bench.py --gpus N` in both its weak (every rank a full batch) and strong (`--scaling strong`: one batch, uneven shards) forms."""
 import os
 import socket
 
@@ -36,15 +37,25 @@ def _worker(rank, world, port, H, ret):
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("H", [24, 5])
-def test_gather_stats_world_size_2_gloo(H):
+def _run(world, H):
     s = socket.socket()
     s.bind(("127.0.0.1", 0))
     port = s.getsockname()[1]
     s.close()
     mgr = mp.Manager()
     ret = mgr.dict()
-    mp.spawn(_worker, args=(2, port, H, ret), nprocs=2, join=True)
+    mp.spawn(_worker, args=(world, port, H, ret), nprocs=world, join=True)
     expect = torch.stack([torch.tensor([1000 + h, 7 * h], dtype=torch.int64) for h in range(H)])[None]
-    for r in range(2):
+    for r in range(world):
         assert torch.equal(ret[r], expect)
+
+
+@pytest.mark.parametrize("H", [24, 5])
+def test_gather_stats_world_size_2_gloo(H):
+    _run(2, H)
+
+
+def test_gather_stats_uneven_strong_scaling_split_40_heads_over_3_ranks():
+    """Config 3's 40 heads over 3 ranks (14 + 13 + 13): the split `bench.py --scaling strong` makes."""
+    assert [shard_heads(40, 3, r) for r in range(3)] == [(0, 14), (14, 27), (27, 40)]
+    _run(3, 40)
