@@ -248,6 +248,26 @@ class Gpu:
         per = [evs[i].elapsed_time(evs[i + 1]) for i in range(steps)]
         return evs[0].elapsed_time(evs[-1]), per, self.stats.cpu().numpy().copy()
 
+    def effective_clock(self, mode, lam):
+        """The SM clock a launch actually runs at, from the kernel's own counters: the debug instantiation sums clock64()
+        cycles over its CTAs (params->cycles_out); with one CTA resident per SM and whole waves, sum / (SMs * time) is the
+        clock.  Called right after a timed loop (chip hot), outside every timed region."""
+        torch = self.torch
+        n_sm = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+        cyc = torch.zeros(2, device="cuda", dtype=torch.int64)
+        p = self.sa.make_params(lam=lam, stream=self.stream.cuda_stream, cycles_out=cyc)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(3):                                    # two to settle, the third is measured
+            if i == 2:
+                e0.record(self.stream)
+            self.sa.sparse_attn_fwd(self.q, self.k, self.v, self.out, self.lse, self.B, self.H, self.N, self.D, p, mode, self.stats)
+        e1.record(self.stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        cycles, ctas = (int(x) for x in cyc.tolist())
+        return {"cta_cycles_sum": cycles, "ctas": ctas, "waves": ctas / n_sm, "debug_launch_ms": ms,
+                "sm_mhz_effective": cycles / (n_sm * ms * 1e3)}
+
     def keep_dense(self):
         self.out_dense, self.lse_dense = self.out.clone(), self.lse.clone()
 
@@ -680,6 +700,8 @@ def main():
             else:
                 st_all = st[None]
             res[mname] = mode_entry(g, BH_total, total / args.steps, per, st_all, st[None])
+            if vi == 0 and mname in ("dense", "dynamic"):
+                res[mname]["clock"] = g.effective_clock(mode, mlam)
             if mname == "dense":
                 g.keep_dense()
             else:
@@ -713,14 +735,22 @@ def main():
 
     sampler.__exit__()
     clocks = sampler.summary()
+    for mname in ("dense", "dynamic"):                       # the clock the kernels' own cycle counters imply, beside the sampled one
+        eff = results.get(variants[0][0], {}).get(mname, {}).get("clock")
+        if eff:
+            clocks["sm_mhz_effective_" + mname] = eff["sm_mhz_effective"]
     if selectors is not None and clocks.get("sm_mhz"):
         # the block-sum pre-pass has one ex2 per logit and no P V to hide it behind: its roofline is the MUFU pipe
         # (16 ex2 / clk / SM, 148 SMs), i.e. 2 D FLOP of Q K^T per ex2; clock = the median sampled in the
         # timed loops of this run
-        peak = 16.0 * 148 * clocks["sm_mhz"] * 1e6 * 2.0 * cfg.D / 1e12
+        # clock: the one DENSE's cycle counters imply in this run (nvidia-smi's sampled value reads higher than the clock
+        # the cycle counts support), else the sampled median
+        mhz = clocks.get("sm_mhz_effective_dense") or clocks["sm_mhz"]
+        peak = 16.0 * 148 * mhz * 1e6 * 2.0 * cfg.D / 1e12
         selectors["block_mass_roofline"] = {"bound": "alu", "pipe": "MUFU ex2, 16 / clk / SM", "achieved": selectors["block_mass_tflops"],
                                             "peak": peak, "unit": "TFLOP/s of Q K^T", "frac": selectors["block_mass_tflops"] / peak,
-                                            "sm_mhz": clocks["sm_mhz"]}
+                                            "sm_mhz": mhz, "sm_mhz_sampled": clocks["sm_mhz"],
+                                            "clock_source": "cycle counters of the DENSE kernel" if clocks.get("sm_mhz_effective_dense") else "nvidia-smi"}
 
     # ------------------------------------------------------------------ end-to-end through the host-buffer C entry point
     qb, kb, vb = host_data[args.config]

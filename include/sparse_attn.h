@@ -78,6 +78,11 @@ typedef struct sparse_attn_params {
                                the mask built).  Debug / parity only. */
     const uint8_t* skip_mask_in; /* MASK mode only (must be NULL otherwise): device, [B, H, T_r, T_c] bytes, non-zero =
                                skip the tile; never written.  Default decision tiles only (tile_q = tile_k = default). */
+    uint64_t* cycles_out;   /* optional, device, uint64[2], overwritten: {sum over the CTAs of the launch of the SM clock
+                               cycles (clock64) each CTA ran, number of CTAs}.  With one CTA resident per SM and a grid of
+                               whole waves, sum / (SM count * kernel time) is the SM clock the launch actually ran at --
+                               measurement support (bench.py), selects the debug instantiation of the kernel; not
+                               supported by sparse_attn_fwd_host (must be NULL there). */
 } sparse_attn_params;
 
 /*

@@ -61,6 +61,7 @@ class SparseAttnParams(ctypes.Structure):
         ("skip_mask_out", ctypes.c_void_p),
         ("margin_out", ctypes.c_void_p),
         ("skip_mask_in", ctypes.c_void_p),
+        ("cycles_out", ctypes.c_void_p),
     ]
 
 
@@ -168,7 +169,7 @@ def _ptr(x) -> Optional[int]:
 
 
 def make_params(lam: float = float("-inf"), softmax_scale: float = 0.0, tile_q: int = 0, tile_k: int = 0,
-                stream=None, skip_mask_out=None, margin_out=None, skip_mask_in=None) -> SparseAttnParams:
+                stream=None, skip_mask_out=None, margin_out=None, skip_mask_in=None, cycles_out=None) -> SparseAttnParams:
     p = SparseAttnParams()
     p.struct_size = ctypes.sizeof(SparseAttnParams)
     p.lambda_ = lam
@@ -179,6 +180,7 @@ def make_params(lam: float = float("-inf"), softmax_scale: float = 0.0, tile_q: 
     p.skip_mask_out = _ptr(skip_mask_out)
     p.margin_out = _ptr(margin_out)
     p.skip_mask_in = _ptr(skip_mask_in)
+    p.cycles_out = _ptr(cycles_out)
     return p
 
 

@@ -56,7 +56,10 @@ constexpr float kRescaleThreshold = 8.0f;
 // N^2 exponentials as the tensor pipe for the MMAs, so every exponential moved off it shortens the softmax phase.
 // Measured on config 1 (steady clocks): 0 / 2 / 3 / 4 of 16 -> DENSE 10.54 / 10.30 / 10.28 / 10.28 ms, FIXED 10.79 / 10.22 /
 // 10.44 / 10.52 ms; 8 of 16 is slower than none (issue slots).
-constexpr int kPolyPairs = 2;
+#ifndef DSA_POLY_PAIRS
+#define DSA_POLY_PAIRS 2                                      // (build-time override for sweeps: -DDSA_POLY_PAIRS=n)
+#endif
+constexpr int kPolyPairs = DSA_POLY_PAIRS;
 static_assert(kPolyPairs >= 0 && kPolyPairs <= 16, "pairs per chunk on the FMA pipe");
 
 struct FwdArgs {
@@ -69,6 +72,7 @@ struct FwdArgs {
     float* mass_out;             // MASS mode: [BH, T_r, T_c] fp32, pre-zeroed: sum over the tile of e^(S - lse)
     float* sqmass_out;           // MASS mode: optional [BH, T_r, T_c] fp32, pre-zeroed: sum over the tile of e^(2 (S - lse))
     const uint8_t* mask_in;      // MASK mode: [BH, T_r, T_c] bytes, non-zero = skip (tile 0 is kept regardless)
+    unsigned long long* cycles;  // debug builds: {sum of clock64 cycles per CTA, CTAs} or null (pre-zeroed)
     int N;
     int T_r;                     // decision tiles along queries
     int T_c;                     // K tiles of BC keys (MMA tiles)
@@ -134,13 +138,15 @@ __device__ __forceinline__ void exp2_poly_x2(uint64_t X, float& p0, float& p1) {
 }
 
 // a5 for 32 columns of one row: P = 2^(s * scale - m) -> 16 packed bf16x2, row sum into the packed pair rs2.
+// kPoly = the number of the chunk's 16 pairs that take the FMA-pipe polynomial (evenly spread among the MUFU ones).
+template <int kPoly = kPolyPairs>
 __device__ __forceinline__ void exp_chunk(const uint32_t (&s)[32], uint64_t scale2, uint64_t negm2, uint64_t& rs2,
                                           uint32_t (&pk)[16]) {
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const uint64_t X = fma_f32x2(pack_f32x2(__uint_as_float(s[2 * i]), __uint_as_float(s[2 * i + 1])), scale2, negm2);
         float p0, p1;
-        if (((i + 1) * kPolyPairs) / 16 > (i * kPolyPairs) / 16) {              // kPolyPairs of the 16 pairs, evenly spread
+        if (((i + 1) * kPoly) / 16 > (i * kPoly) / 16) {                        // kPoly of the 16 pairs, evenly spread
             exp2_poly_x2(X, p0, p1);
         } else {
             float x0, x1;
@@ -259,6 +265,8 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr;
+    long long cta_t0 = 0;                                    // (debug builds: SM cycles of this CTA, for the effective clock)
+    if (kDebug && threadIdx.x == 0 && a.cycles) cta_t0 = clock64();
 
     if (warp >= 8) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsOther));
@@ -1088,6 +1096,10 @@ sparse_attn_fwd_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_co
     tc_fence_before();
     __syncthreads();
     if (warp == kMmaWarp0) tmem_dealloc(tmem_base, kTmemCols);
+    if (kDebug && threadIdx.x == 0 && a.cycles) {
+        atomicAdd(a.cycles, static_cast<unsigned long long>(clock64() - cta_t0));
+        atomicAdd(a.cycles + 1, 1ull);
+    }
 }
 
 }  // namespace dsa

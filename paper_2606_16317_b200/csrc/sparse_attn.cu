@@ -98,6 +98,7 @@ struct Resolved {
     uint8_t* skip_mask;
     float* margin;
     const uint8_t* mask_in;
+    uint64_t* cycles;
 };
 
 // Host-side validation shared by the device and host-buffer entry points.
@@ -119,6 +120,7 @@ int validate(const void* q, const void* k, const void* v, void* out, int B, int 
     r->skip_mask = nullptr;
     r->margin = nullptr;
     r->mask_in = nullptr;
+    r->cycles = nullptr;
     if (p) {
         if (p->struct_size != sizeof(sparse_attn_params))
             return fail(SPARSE_ATTN_ERR_PARAMS, "params->struct_size = %u, expected %zu", p->struct_size, sizeof(sparse_attn_params));
@@ -151,6 +153,7 @@ int validate(const void* q, const void* k, const void* v, void* out, int B, int 
             return fail(SPARSE_ATTN_ERR_PARAMS, "skip_mask_in is set but mode %d is not MASK", mode);
         }
         r->mask_in = p->skip_mask_in;
+        r->cycles = p->cycles_out;
     }
     return 0;
 }
@@ -289,6 +292,7 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     a.skip_mask = r.skip_mask;
     a.margin = r.margin;
     a.mask_in = r.mask_in;
+    a.cycles = reinterpret_cast<unsigned long long*>(r.cycles);
     a.N = N;
     a.T_r = (N + r.tile_q - 1) / r.tile_q;
     a.T_c = (N + mma_k - 1) / mma_k;
@@ -299,8 +303,9 @@ int sparse_attn_fwd(const void* q, const void* k, const void* v, void* out, floa
     a.lambda_log2 = r.lambda * dsa::kLog2e;
 
     if (stats_out) CUDA_TRY(cudaMemsetAsync(stats_out, 0, sizeof(int64_t) * 2 * BH, r.stream));
+    if (r.cycles) CUDA_TRY(cudaMemsetAsync(r.cycles, 0, sizeof(uint64_t) * 2, r.stream));
     const bool sparse = mode != SPARSE_ATTN_DENSE;
-    const bool debug = r.skip_mask || r.margin;
+    const bool debug = r.skip_mask || r.margin || r.cycles;
     if (D == 128) {
         if (!sparse && !debug) return launch<128, 128, 1, DSA_NK, DSA_NV, false, false>(tq, tk, tv, a, BH, r.stream);
         if (!sparse) return launch<128, 128, 1, DSA_NK, DSA_NV, false, true>(tq, tk, tv, a, BH, r.stream);
@@ -333,6 +338,7 @@ int sparse_attn_fwd_host(const void* q, const void* k, const void* v, void* out,
     int rc = validate(q, k, v, out, B, H, N, D, params, mode, &r);
     if (rc) return rc;
     if ((rc = check_device())) return rc;
+    if (r.cycles) return fail(SPARSE_ATTN_ERR_PARAMS, "params->cycles_out is not supported by the host-buffer entry");
     const size_t BH = static_cast<size_t>(B) * H;
     const size_t head_elems = static_cast<size_t>(N) * D;
     const size_t T_r = (N + r.tile_q - 1) / r.tile_q, T_c = (N + r.tile_k - 1) / r.tile_k;

@@ -38,10 +38,11 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_params_struct_matches_header_layout():
-    # uint32, float, float, int32, int32, (pad), void*, uint8_t*, float*, const uint8_t*
-    assert ctypes.sizeof(sa.SparseAttnParams) == 56
+    # uint32, float, float, int32, int32, (pad), void*, uint8_t*, float*, const uint8_t*, uint64_t*
+    assert ctypes.sizeof(sa.SparseAttnParams) == 64
     assert sa.SparseAttnParams.stream.offset == 24
     assert sa.SparseAttnParams.skip_mask_in.offset == 48
+    assert sa.SparseAttnParams.cycles_out.offset == 56
 
 
 def test_lambda_helpers():
