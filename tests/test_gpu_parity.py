@@ -334,3 +334,33 @@ def test_repeated_launches_are_bit_identical(parity, seed, tile_k):
         np.testing.assert_array_equal(again.out, first.out)
         np.testing.assert_array_equal(again.lse, first.lse)
     torch.cuda.synchronize()
+
+
+def test_cycle_counters_of_the_debug_instantiation(parity, seed):
+    """params->cycles_out (measurement support of bench.py): {sum of per-CTA clock64 cycles, CTAs of the launch}; the
+    buffer is overwritten on every call, selecting the debug instantiation changes no result, and the host-buffer entry
+    refuses it."""
+    import torch
+
+    import paper_2606_16317_b200 as sa
+    for name in ("cfg0",):
+        cfg = CONFIGS[name]
+        q, k, v = make_qkv(cfg, seed)
+        dq, dk, dv = (parity.to_dev_bf16(np.ascontiguousarray(x)) for x in (q, k, v))
+        out = torch.empty_like(dq)
+        ref = torch.empty_like(dq)
+        cyc = torch.full((2,), 12345, device="cuda", dtype=torch.int64)
+        ctas_per_head = (-(-cfg.N // 128) + 1) // 2                       # two 128-row MMA tiles per CTA
+        for mode, lam in ((MODE_DENSE, -math.inf), (MODE_DYNAMIC, -3.0)):
+            sa.sparse_attn_fwd(dq, dk, dv, ref, None, cfg.B, cfg.H, cfg.N, cfg.D, sa.make_params(lam=lam), mode, None)
+            for _ in range(2):
+                sa.sparse_attn_fwd(dq, dk, dv, out, None, cfg.B, cfg.H, cfg.N, cfg.D, sa.make_params(lam=lam, cycles_out=cyc), mode, None)
+                torch.cuda.synchronize()
+                cycles, ctas = cyc.tolist()
+                assert ctas == cfg.B * cfg.H * ctas_per_head
+                assert 1000 * ctas < cycles < 10 ** 9 * ctas
+            assert torch.equal(out.view(torch.int16), ref.view(torch.int16))
+    with pytest.raises(sa.SparseAttnError) as e:
+        sa.sparse_attn_fwd_host(q, k, v, np.zeros_like(q), None, cfg.B, cfg.H, cfg.N, cfg.D, sa.make_params(lam=-3.0, cycles_out=cyc),
+                                MODE_DYNAMIC, None)
+    assert e.value.status == -6
